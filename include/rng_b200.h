@@ -1,0 +1,187 @@
+/*
+ * rng_b200.h -- C-ABI boundary of the B200-native (sm_100a) implementation of
+ * the hot path of Manssen, Weigel & Hartmann, "Random number generators for
+ * massively parallel simulations on GPU" (arXiv:1204.6193):
+ *
+ *     many independent per-thread pseudo-random streams, seeded and advanced in
+ *     parallel, their output either written in bulk to HBM or
+ *     drawn in-register by a consumer kernel, the consumer
+ *     being the checkerboard Metropolis sweep of the 2D Ising model the paper
+ *     uses as its application test.
+ *
+ * Citations are lines of /root/reference/PAPER.md ("PAPER.md:<line>") or a
+ * reading listed in DESIGN.md section 3 ("R-<id>").
+ *
+ * General conventions
+ * -------------------
+ *  - Every function returns RNG_OK (0) or a negative error code; nothing throws,
+ *    aborts or prints.  rng_last_error() returns a thread-local message for the
+ *    last failing call of the calling thread.
+ *  - Pointers named d_* are DEVICE pointers owned by the caller (e.g. PyTorch
+ *    tensors), 16-byte aligned unless stated, on the device that was current
+ *    when the handle was created.  Pointers named h_* are HOST pointers owned by
+ *    the caller (pinned memory makes the copies asynchronous, pageable works).
+ *    The library never allocates or frees caller buffers.
+ *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default
+ *    stream).  Device-pointer calls only enqueue work and return without
+ *    synchronising.  Host-pointer calls (`*_host`) return after the result is
+ *    in the host buffer.
+ *  - A handle owns its generator state (device memory).  All streams of a handle
+ *    advance in lockstep: every call consumes the same number of draws from
+ *    every stream, and successive calls CONTINUE the streams:
+ *    fill(n) followed by fill(m) produces exactly what fill(n+m) would.
+ *  - Canonical output layout is stream-major:  out[s*n + j] = draw j (of this
+ *    call) of local stream s  (BASELINE.json config 1: "per stream to a flat
+ *    array").
+ *  - No CPU fallback exists: without a CUDA device every call that needs one
+ *    fails with RNG_E_CUDA.
+ */
+#ifndef RNG_B200_H
+#define RNG_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rng_handle rng_handle; /* opaque */
+
+/* Generator kinds.  Stream s below is the GLOBAL stream id (first + local index);
+ * SM_seed[k] is the k-th (0-based) output of splitmix64 started at `seed` (R-S1). */
+enum {
+    /* x <- a x + c mod 2^64, a = 2862933555777941757, c = 1442695040888963407
+     * (eq.(1), :46); draw j = 32 most significant bits of x_j
+     * (R-A3: output, then advance); x_0 of stream s = SM_seed[s]
+     * ("random" seeding). */
+    RNG_LCG64 = 0,
+    /* the paper's sub-stream method (eq.(2),(3)): ONE global
+     * sequence X_0 = SM_seed[0], stream s draw j = hi32(X_{s + j*n_total}). */
+    RNG_LCG64_LEAPFROG = 1,
+    /* Marsaglia's XORWOW (recurrence of Ref.[30], R-B1):
+     * t=x^(x>>2); x=y; y=z; z=w; w=v; v=(v^(v<<4))^(t^(t<<1)); d+=362437;
+     * return d+v.  Seeding: (x,y),(z,w),(v,d) = (lo32,hi32) of SM_seed[3s],
+     * SM_seed[3s+1], SM_seed[3s+2]; if x|y|z|w|v == 0 then v = 1 (R-B2, R-B3). */
+    RNG_XORWOW = 2,
+    /* Philox4x32-10 (constants of Ref.[20], R-C1).  Key =
+     * s XOR seed (64 bit, low word = k0); counter = (lo32(b), hi32(b), 0, 0) with
+     * b = floor(j/4) the 4-word block index over the handle's lifetime; draw j
+     * is word j mod 4 of that block (BASELINE.json config 2, R-C2).  Stateless. */
+    RNG_PHILOX4X32_10 = 3,
+    /* The paper's XORShift1024/Weyl generator (eq.(8), :177,
+     * :201-225 Listing 1, :232-240).  One 1024-bit instance per WARP: streams
+     * 32g..32g+31 are the 32 words of instance g, word 0 most significant
+     * (R-D1, R-D4).  Update X ^= X<<329; X ^= X>>347; X ^= X<<344 (zeros shift
+     * in); output of the n-th update since creation: (y ^ (y>>16)) + x_word with
+     * y = n*362437 mod 2^32 (R-D6).  Seeding ("sloppy" variant, PAPER.md:230,
+     * R-D7): words 2k, 2k+1 of instance g = lo32, hi32 of SM_seed[16g+k]; an
+     * all-zero instance gets word 31 = 1.  n_streams and first must be
+     * multiples of 32. */
+    RNG_XS1024W = 4
+};
+
+enum {
+    RNG_OK = 0,
+    RNG_E_INVAL = -1,       /* bad argument (null, misaligned, size constraint)   */
+    RNG_E_NOMEM = -2,       /* host or device allocation failed                   */
+    RNG_E_CUDA = -3,        /* CUDA runtime error, or no device                   */
+    RNG_E_UNSUPPORTED = -4  /* valid request the library does not implement       */
+};
+
+/* ---- a1: seeding / stream setup --------------
+ * rng_create: streams [0, n_streams) of n_streams.  Runs the seeding kernel on
+ * the current device (legacy default stream, synchronised before returning).
+ * rng_create_shard: local streams are the global streams [first, first+n_local)
+ * out of n_total (for one-process-per-GPU sharding; n_total only matters for
+ * RNG_LCG64_LEAPFROG, where it is the stride of the global sequence).
+ * Errors: RNG_E_INVAL (n == 0, range overflow, XS1024W not in whole instances,
+ * unknown kind, out == NULL), RNG_E_NOMEM, RNG_E_CUDA. */
+int rng_create(int kind, uint64_t n_streams, uint64_t seed, rng_handle **out);
+int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_local,
+                     uint64_t seed, rng_handle **out);
+/* frees the state; NULL is allowed */
+int rng_destroy(rng_handle *h);
+
+/* ---- a2-a5,a7: fill mode -------------------------------------------------------
+ * d_out[s*n + j] = draw (draws_done + j) of local stream s, s < n_local, j < n;
+ * then draws_done += n.  n == 0 is a no-op.  d_out must hold n_local*n elements
+ * and be 16-byte aligned (else RNG_E_INVAL).  Any n is accepted; n % 4 == 0 (and,
+ * for Philox, draws_done % 4 == 0) takes the 128-bit-store path. */
+int rng_fill_u32(rng_handle *h, uint32_t *d_out, uint64_t n, void *cuda_stream);
+/* same stream pushed through the fixed map f = (float)(u >> 8) * 2^-24, exact,
+ * in [0, 1 - 2^-24]  (BASELINE.json; the paper's u = x/m is PAPER.md:35, R-A4) */
+int rng_fill_f32(rng_handle *h, float *d_out, uint64_t n, void *cuda_stream);
+
+/* ---- a6: in-register draw mode -------------------------------------------------
+ * Each stream draws n numbers that never leave the register file and reduces
+ * them: d_out[2s] = XOR_j u_{s,j}, d_out[2s+1] = SUM_j u_{s,j} mod 2^32.
+ * d_out holds 2*n_local uint32, 8-byte aligned.  draws_done += n.
+ * (This is the mode of the paper's peak numbers.) */
+int rng_draw_reduce(rng_handle *h, uint32_t *d_out, uint64_t n, void *cuda_stream);
+
+/* ---- a8: consumer: checkerboard Metropolis sweeps of the 2D Ising model --------
+ * (BASELINE.json config 5; R-E1..E8.)
+ * d_spins: int8 +1/-1, row-major L x L, periodic; L even, >= 4.  Colour of (x,y)
+ * is (x+y)&1; a sweep is the colour-0 half-sweep then the colour-1 half-sweep.
+ * Sites of one colour are numbered q = y*(L/2) + xh with x = 2*xh + ((y+c)&1).
+ * With S = n_local streams, K = (L*L/2)/S (S must divide L*L/2): stream s owns
+ * q in [sK,(s+1)K) of both colours, visits them in increasing q and spends ONE
+ * draw on each, accepted or not:  h = spin * (sum of its 4 neighbours);
+ * flip iff (float)(r>>8)*2^-24 < P[(h+4)/2], P[i] = (float)exp(-2.0*beta*(2i-4))
+ * evaluated in double on the host and rounded to float (strict <).
+ * Equivalent to: per half-sweep, fill K draws per stream, then apply.
+ * draws_done += 2*K*n_sweeps.  d_energy_trace: NULL, or int64[n_sweeps] (device)
+ * receiving E = -sum_<ij> s_i s_j after every sweep.  Every kind is supported. */
+int ising_sweep(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_t n_sweeps,
+                int64_t *d_energy_trace, void *cuda_stream);
+
+/* helpers (not hot path) */
+/* spin i = +1 if bit (i & 63) of SM_seed[i >> 6] is set, else -1 */
+int ising_init_random(int8_t *d_spins, uint32_t L, uint64_t seed, void *cuda_stream);
+/* *d_out = E = -sum over bonds s_i s_j, each bond once, periodic */
+int ising_energy(const int8_t *d_spins, uint32_t L, int64_t *d_out, void *cuda_stream);
+/* the acceptance table the sweep uses, as integers T[i] = min(2^24, ceil(P[i]*2^24)):
+ * (r>>8) < T[i]  <=>  (float)(r>>8)*2^-24 < P[i]  exactly.  P_out / T_out may be NULL. */
+int ising_accept_table(double beta, float P_out[5], uint32_t T_out[5]);
+
+/* ---- host-buffer entry points (end-to-end path) -------------------------------
+ * Same results as the calls above, but the caller's buffers are HOST memory:
+ * the library stages through device memory it owns (grown on demand, freed by
+ * rng_destroy), overlaps kernels with the device->host copies in chunks, and
+ * returns when the host buffer is complete. */
+int rng_fill_u32_host(rng_handle *h, uint32_t *h_out, uint64_t n, void *cuda_stream);
+int rng_fill_f32_host(rng_handle *h, float *h_out, uint64_t n, void *cuda_stream);
+int rng_draw_reduce_host(rng_handle *h, uint32_t *h_out, uint64_t n, void *cuda_stream);
+/* h_spins is copied to the device, swept, and copied back; h_energy_trace may be NULL */
+int ising_sweep_host(rng_handle *h, int8_t *h_spins, uint32_t L, double beta, uint32_t n_sweeps,
+                     int64_t *h_energy_trace, void *cuda_stream);
+
+/* ---- state access (checkpoint / resume; the state is stored to
+ * global memory after every kernel and reloaded by the next) --------------------
+ * Canonical order, independent of the device layout:
+ *   LCG64 / LEAPFROG: n_local x u64 (current x of each stream)
+ *   XORWOW: n_local x {x,y,z,w,v,d} u32, stream-major
+ *   PHILOX: 0 bytes;  XS1024W: n_local x u32 (word s%32 of instance s/32)
+ * rng_get_state/rng_set_state synchronise the device; bytes must equal
+ * rng_state_bytes(kind, n_local).  draws_done is read / set separately. */
+uint64_t rng_state_bytes(int kind, uint64_t n_streams);
+int rng_get_state(rng_handle *h, void *h_buf, uint64_t bytes);
+int rng_set_state(rng_handle *h, const void *h_buf, uint64_t bytes);
+uint64_t rng_draws_done(const rng_handle *h);
+int rng_set_draws_done(rng_handle *h, uint64_t draws_done);
+
+/* kernel-variant selection for measurements: name in {"xs1024", "ising", "store"},
+ * value = variant index (0 = default).  Every variant of an operation produces
+ * identical bits; see DESIGN.md section 6.  Unknown name/value: RNG_E_INVAL. */
+int rng_set_variant(rng_handle *h, const char *name, int value);
+
+/* number of kernels launched by this library in the calling process so far */
+uint64_t rng_kernel_launches(void);
+const char *rng_last_error(void);
+/* "rng_b200 <version> sm_100a" */
+const char *rng_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RNG_B200_H */

@@ -1,0 +1,93 @@
+// draw.cu -- in-register draw mode: every stream draws n numbers
+// that never leave the register file and reduces them to {XOR, SUM mod 2^32}.  This is the
+// regime of the paper's peak numbers ("compute-bound"): the only memory
+// traffic is one state load and one state store per stream plus 8 bytes out.
+#include "internal.h"
+#include "streams.cuh"
+
+namespace rngb200 {
+
+template <int KIND>
+__global__ void __launch_bounds__(256) draw_reduce_kernel(Gen g, uint2 *__restrict__ out, uint64_t n)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= g.S) return; // xs1024: S % 32 == 0, whole warps leave together
+    Stream<KIND> gen;
+    gen.load(g, s);
+    uint32_t x = 0u, sum = 0u;
+    uint64_t j = 0;
+    for (; j + 4 <= n; j += 4) {
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const uint32_t u = gen.next();
+            x ^= u;
+            sum += u;
+        }
+    }
+    for (; j < n; j++) {
+        const uint32_t u = gen.next();
+        x ^= u;
+        sum += u;
+    }
+    gen.store(g, s);
+    out[s] = make_uint2(x, sum);
+}
+
+// Philox: counter-based, so the n draws of a stream are the words of consecutive blocks;
+// whole blocks are reduced four words at a time with the round keys' base hoisted.
+__global__ void __launch_bounds__(256) philox_draw_reduce_kernel(Gen g, uint2 *__restrict__ out, uint64_t n)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= g.S) return;
+    const uint64_t key = (g.first + s) ^ g.seed;
+    const uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
+    uint64_t j = g.draws_done;
+    const uint64_t end = j + n;
+    uint32_t x = 0u, sum = 0u;
+    // head: words of a partially consumed block
+    if ((j & 3ull) && j < end) {
+        const uint64_t b = j >> 2;
+        const uint4 r = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+        const uint32_t w[4] = {r.x, r.y, r.z, r.w};
+        for (; (j & 3ull) && j < end; j++) {
+            x ^= w[j & 3ull];
+            sum += w[j & 3ull];
+        }
+    }
+    for (; j + 4 <= end; j += 4) {
+        const uint64_t b = j >> 2;
+        const uint4 r = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+        x ^= r.x ^ r.y ^ r.z ^ r.w;
+        sum += r.x + r.y + r.z + r.w;
+    }
+    if (j < end) { // tail
+        const uint64_t b = j >> 2;
+        const uint4 r = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+        const uint32_t w[4] = {r.x, r.y, r.z, r.w};
+        for (; j < end; j++) {
+            x ^= w[j & 3ull];
+            sum += w[j & 3ull];
+        }
+    }
+    out[s] = make_uint2(x, sum);
+}
+
+cudaError_t launch_draw_reduce(const rng_handle &h, uint32_t *d_out, uint64_t n, cudaStream_t st)
+{
+    const Gen &g = h.g;
+    const uint64_t grid = (g.S + 255) / 256;
+    if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+    uint2 *o = (uint2 *)d_out;
+    switch (g.kind) {
+    case RNG_LCG64: draw_reduce_kernel<RNG_LCG64><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_LCG64_LEAPFROG: draw_reduce_kernel<RNG_LCG64_LEAPFROG><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_XORWOW: draw_reduce_kernel<RNG_XORWOW><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_XS1024W: draw_reduce_kernel<RNG_XS1024W><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_PHILOX4X32_10: philox_draw_reduce_kernel<<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    default: return cudaErrorInvalidValue;
+    }
+    count_launch();
+    return cudaGetLastError();
+}
+
+} // namespace rngb200

@@ -1,0 +1,68 @@
+// internal.h -- handle layout and the launch functions the C-ABI (api.cu) calls.
+// Product code (sm_100a); shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/rng_b200.h"
+#include "generators.cuh"
+
+namespace rngb200 {
+
+// Device-side LCG table built by the seeding kernel (eq.(2)):
+//   pow2[m]  = step^(2^m),  m = 0..63     (pow2[0] is the per-draw step map itself)
+//   mult4[t] = step^(4 t),  t = 0..255    (lane offsets of the intra-stream leapfrog)
+// where step = (a, c) for RNG_LCG64 and (a, c)^n_total for RNG_LCG64_LEAPFROG.
+struct LcgTable {
+    Affine pow2[64];
+    Affine mult4[256];
+};
+
+// Device state layout (all coalesced for "thread s handles stream s"):
+//   LCG64 / LEAPFROG : u64 x[S]
+//   XORWOW           : u32 w[6][S]   (word k of stream s at w[k*S + s]; k = x,y,z,w,v,d)
+//   PHILOX           : none
+//   XS1024W          : u32 w[S]      (word `lane` of instance g at w[32 g + lane])
+struct Gen {
+    int kind;
+    uint64_t S;          // local streams
+    uint64_t first;      // global id of local stream 0
+    uint64_t n_total;    // global number of streams
+    uint64_t seed;
+    uint64_t draws_done; // per stream, all streams in lockstep
+    void *state;         // device
+    const LcgTable *lcg; // device (LCG kinds only)
+};
+
+} // namespace rngb200
+
+struct rng_handle {
+    rngb200::Gen g;
+    int device;
+    uint64_t state_bytes;
+    void *staging;          // device staging for the *_host entry points
+    uint64_t staging_bytes;
+    int64_t *energy_scratch; // device, 1 x int64
+    int var_xs1024, var_ising, var_store;
+};
+
+namespace rngb200 {
+
+void count_launch(uint64_t n = 1);
+
+// seed.cu
+cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st);
+// fill.cu  (f32 = apply the (u>>8)*2^-24 map; out is uint32_t* or float*)
+cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st);
+// draw.cu
+cudaError_t launch_draw_reduce(const rng_handle &h, uint32_t *d_out, uint64_t n, cudaStream_t st);
+// ising.cu
+struct IsingTable {
+    uint32_t T[5]; // integer thresholds: (r>>8) < T[i]  <=>  u < P[i]
+};
+cudaError_t launch_ising_half_sweep(const rng_handle &h, int8_t *d_spins, uint32_t L, const IsingTable &tab,
+                                    uint64_t K, uint64_t draws_done, int colour, cudaStream_t st);
+cudaError_t launch_ising_init_random(int8_t *d_spins, uint32_t L, uint64_t seed, cudaStream_t st);
+cudaError_t launch_ising_energy(const int8_t *d_spins, uint32_t L, int64_t *d_out, cudaStream_t st);
+
+} // namespace rngb200

@@ -1,0 +1,118 @@
+// seed.cu -- a1: seeding / stream-setup kernels.
+//
+// PAPER.md:21 lists the three ways to get independent streams; the graded path uses
+// (2) "random seeding from another RNG" with splitmix64 as that
+// RNG (BASELINE.json configs), (1) skip-ahead for the LCG leapfrog kind (PAPER.md:39-46,
+// eq.(2),(3)) and (3) distinct keys for Philox (nothing to store).
+// splitmix64 is random-access in the stream id, so every thread seeds its own stream.
+#include "internal.h"
+
+namespace rngb200 {
+
+// One CTA of 256 threads builds the LCG table (see LcgTable in internal.h).
+// step = (a,c)^stride by binary exponentiation; pow2 by repeated squaring; mult4[t] =
+// step^(4t) by binary exponentiation over the bits of 4t using pow2.
+__global__ void __launch_bounds__(256) lcg_table_kernel(LcgTable *tab, uint64_t stride)
+{
+    __shared__ Affine pw[64];
+    if (threadIdx.x == 0) {
+        Affine p = affine_pow(Affine{kLcgA, kLcgC}, stride);
+        for (int m = 0; m < 64; m++) {
+            pw[m] = p;
+            tab->pow2[m] = p;
+            p = affine_compose(p, p);
+        }
+    }
+    __syncthreads();
+    const uint32_t e = 4u * threadIdx.x; // < 1024: bits 2..9
+    Affine r{1ull, 0ull};
+#pragma unroll
+    for (int m = 2; m < 10; m++)
+        if ((e >> m) & 1u) r = affine_compose(pw[m], r);
+    tab->mult4[threadIdx.x] = r;
+}
+
+// RNG_LCG64: x_0 of stream s = SM_seed[s]  ("random" seeding)
+__global__ void seed_lcg64_kernel(uint64_t *x, uint64_t S, uint64_t first, uint64_t seed)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < S) x[s] = splitmix64_at(seed, first + s);
+}
+
+// RNG_LCG64_LEAPFROG: one global sequence X_0 = SM_seed[0]; stream s starts at X_s =
+// (a,c)^s applied to X_0 -- eq.(2) with t = s, by binary exponentiation.
+__global__ void seed_lcg64_leapfrog_kernel(uint64_t *x, uint64_t S, uint64_t first, uint64_t seed)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    const Affine j = affine_pow(Affine{kLcgA, kLcgC}, first + s);
+    x[s] = affine_apply(j, splitmix64_at(seed, 0));
+}
+
+// RNG_XORWOW (R-B2, R-B3): three splitmix64 outputs per stream, interleaved layout.
+__global__ void seed_xorwow_kernel(uint32_t *w, uint64_t S, uint64_t first, uint64_t seed)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    const uint64_t g = first + s;
+    const uint64_t z0 = splitmix64_at(seed, 3 * g), z1 = splitmix64_at(seed, 3 * g + 1),
+                   z2 = splitmix64_at(seed, 3 * g + 2);
+    uint32_t x = (uint32_t)z0, y = (uint32_t)(z0 >> 32), z = (uint32_t)z1, ww = (uint32_t)(z1 >> 32),
+             v = (uint32_t)z2, d = (uint32_t)(z2 >> 32);
+    if ((x | y | z | ww | v) == 0u) v = 1u; // the all-zero xorshift state is a fixed point
+    w[0 * S + s] = x;
+    w[1 * S + s] = y;
+    w[2 * S + s] = z;
+    w[3 * S + s] = ww;
+    w[4 * S + s] = v;
+    w[5 * S + s] = d;
+}
+
+// RNG_XS1024W ("sloppy" seeding, R-D7): words 2k, 2k+1 of instance g are
+// lo32, hi32 of SM_seed[16 g + k].  One warp per instance; blockDim is a multiple of 32.
+__global__ void seed_xs1024_kernel(uint32_t *w, uint64_t S, uint64_t first, uint64_t seed)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= S) return; // S % 32 == 0: whole warps leave together
+    const uint64_t gs = first + s, g = gs >> 5;
+    const uint32_t lane = (uint32_t)(gs & 31u);
+    const uint64_t z = splitmix64_at(seed, 16 * g + (lane >> 1));
+    uint32_t word = (lane & 1u) ? (uint32_t)(z >> 32) : (uint32_t)z;
+    const bool all_zero = !__any_sync(0xffffffffu, word != 0u);
+    if (all_zero && lane == 31u) word = 1u; // zero is a fixed point of the linear map
+    w[s] = word;
+}
+
+void count_launch(uint64_t n);
+
+cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st)
+{
+    const unsigned B = 256;
+    const unsigned grid = (unsigned)((g.S + B - 1) / B);
+    switch (g.kind) {
+    case RNG_LCG64:
+        lcg_table_kernel<<<1, 256, 0, st>>>(tab, 1);
+        seed_lcg64_kernel<<<grid, B, 0, st>>>((uint64_t *)g.state, g.S, g.first, g.seed);
+        count_launch(2);
+        break;
+    case RNG_LCG64_LEAPFROG:
+        lcg_table_kernel<<<1, 256, 0, st>>>(tab, g.n_total);
+        seed_lcg64_leapfrog_kernel<<<grid, B, 0, st>>>((uint64_t *)g.state, g.S, g.first, g.seed);
+        count_launch(2);
+        break;
+    case RNG_XORWOW:
+        seed_xorwow_kernel<<<grid, B, 0, st>>>((uint32_t *)g.state, g.S, g.first, g.seed);
+        count_launch();
+        break;
+    case RNG_XS1024W:
+        seed_xs1024_kernel<<<grid, B, 0, st>>>((uint32_t *)g.state, g.S, g.first, g.seed);
+        count_launch();
+        break;
+    case RNG_PHILOX4X32_10:
+    default:
+        break; // key = s ^ seed and counter = draw index are intrinsic: nothing to set up
+    }
+    return cudaGetLastError();
+}
+
+} // namespace rngb200

@@ -1,0 +1,114 @@
+// streams.cuh -- "thread s owns stream s" generator objects: state in registers, loaded
+// from / stored to the handle's interleaved device state with coalesced accesses
+// (PAPER.md:19 requirement (b), :58).
+// Product code (sm_100a); shares nothing with oracle/.
+#pragma once
+#include "internal.h"
+
+namespace rngb200 {
+
+template <int KIND>
+struct Stream;
+
+// ---- LCG64 and its leapfrog sub-streams: x, and the handle's step map (pow2[0]) ----
+struct StreamLcg {
+    uint64_t x;
+    Affine step;
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s)
+    {
+        x = ((const uint64_t *)g.state)[s];
+        step = g.lcg->pow2[0];
+    }
+    __device__ __forceinline__ uint32_t next()
+    {
+        const uint32_t r = (uint32_t)(x >> 32); // 32 most significant bits
+        x = step.A * x + step.C;                // eq.(1) / eq.(2)
+        return r;
+    }
+    __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint64_t *)g.state)[s] = x; }
+};
+template <>
+struct Stream<RNG_LCG64> : StreamLcg {
+};
+template <>
+struct Stream<RNG_LCG64_LEAPFROG> : StreamLcg {
+};
+
+// ---- XORWOW: six words, interleaved w[k*S + s] ----
+template <>
+struct Stream<RNG_XORWOW> {
+    Xorwow st;
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s)
+    {
+        const uint32_t *w = (const uint32_t *)g.state;
+        st.x = w[0 * g.S + s];
+        st.y = w[1 * g.S + s];
+        st.z = w[2 * g.S + s];
+        st.w = w[3 * g.S + s];
+        st.v = w[4 * g.S + s];
+        st.d = w[5 * g.S + s];
+    }
+    __device__ __forceinline__ uint32_t next() { return st.next(); }
+    __device__ __forceinline__ void store(const Gen &g, uint64_t s)
+    {
+        uint32_t *w = (uint32_t *)g.state;
+        w[0 * g.S + s] = st.x;
+        w[1 * g.S + s] = st.y;
+        w[2 * g.S + s] = st.z;
+        w[3 * g.S + s] = st.w;
+        w[4 * g.S + s] = st.v;
+        w[5 * g.S + s] = st.d;
+    }
+};
+
+// ---- Philox4x32-10: key = global stream id ^ seed; position = draws_done (R-C2) ----
+template <>
+struct Stream<RNG_PHILOX4X32_10> {
+    uint32_t k0, k1;
+    uint64_t j; // next draw index
+    uint4 buf;
+    __device__ __forceinline__ void refill()
+    {
+        const uint64_t b = j >> 2;
+        buf = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+    }
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s)
+    {
+        const uint64_t key = (g.first + s) ^ g.seed;
+        k0 = (uint32_t)key;
+        k1 = (uint32_t)(key >> 32);
+        j = g.draws_done;
+        if (j & 3ull) refill();
+    }
+    __device__ __forceinline__ uint32_t next()
+    {
+        const uint32_t p = (uint32_t)j & 3u;
+        if (p == 0u) refill();
+        j++;
+        return p == 0u ? buf.x : p == 1u ? buf.y : p == 2u ? buf.z : buf.w;
+    }
+    __device__ __forceinline__ void store(const Gen &, uint64_t) {}
+};
+
+// ---- XORShift1024/Weyl, cooperative: lane = word index; whole warps only ----
+template <>
+struct Stream<RNG_XS1024W> {
+    uint32_t s_word;
+    uint32_t n; // low 32 bits of the update count (the Weyl term only needs n mod 2^32)
+    int lane;
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s)
+    {
+        s_word = ((const uint32_t *)g.state)[s];
+        n = (uint32_t)g.draws_done;
+        lane = (int)(threadIdx.x & 31u); // blockDim.x % 32 == 0 and (first + s) % 32 == lane
+    }
+    __device__ __forceinline__ uint32_t next()
+    {
+        s_word = xs1024_update_coop(s_word, lane);
+        n++;
+        return xs1024_weyl_term(n) + s_word;
+    }
+    __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint32_t *)g.state)[s] = s_word; }
+};
+
+} // namespace rngb200
