@@ -1,0 +1,68 @@
+"""BASELINE.json configs C1-C5 as plain data (sizes, seeds, shapes).
+
+This module holds NONE of the method's arithmetic: every input of this hot path is a
+(kind, n_streams, seed, n) tuple or a lattice drawn from a seed by a counter-based
+rule that the oracle and the CUDA path each implement for themselves.  tests/,
+bench.py and __graft_entry__.py read their workload definitions from here.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W = range(5)
+MASTER_SEED = 1                    # "seeded via splitmix64(master seed 1)" (config 1)
+LATTICE_SEED = 2                   # ising_init_random seed
+BETA_C = 0.44068679350977147       # ln(1+sqrt 2)/2 as a double (config 5)
+
+
+@dataclass(frozen=True)
+class FillCfg:
+    name: str
+    kind: int
+    n_streams: int
+    n_per_stream: int          # per call
+    calls: int = 1             # successive calls into one reused buffer (state persists)
+    seed: int = MASTER_SEED
+
+    @property
+    def draws_per_call(self) -> int:
+        return self.n_streams * self.n_per_stream
+
+
+@dataclass(frozen=True)
+class IsingCfg:
+    name: str
+    kind: int
+    L: int
+    beta: float
+    n_streams: int
+    n_sweeps: int
+    seed: int = MASTER_SEED
+    lattice_seed: int = LATTICE_SEED
+
+
+# C1: 64-bit LCG, 1024 streams x 4096 u32 (16 MiB) -- the small case the oracle does in ms
+C1 = FillCfg("C1_lcg64_1024x4096", LCG64, 1024, 4096)
+# C2: Philox4x32-10, 2^20 streams x 1024 u32 = 4 GiB -- the config `metric` is quoted on
+C2 = FillCfg("C2_philox_2^20x1024", PHILOX4X32_10, 1 << 20, 1024)
+# C3: XORWOW, 2^22 threads x 256 draws in-register, {xor,sum} checksum per thread
+C3 = FillCfg("C3_xorwow_2^22x256", XORWOW, 1 << 22, 256)
+# C4: the paper's generator, 2^16 blocks x 256 threads = 2^24 streams x 4096 u32.
+# 256 GiB of output cannot be resident: fill mode = 64 calls x 64 draws into one 4 GiB buffer.
+C4_FILL = FillCfg("C4_xs1024_2^24x4096_fill", XS1024W, 1 << 24, 64, calls=64)
+C4_DRAW = FillCfg("C4_xs1024_2^24x4096_draw", XS1024W, 1 << 24, 4096)
+# supplementary 4 GiB fills for the stateful per-thread generators (SURVEY.md 8(d) C1 note)
+C1_BIG = FillCfg("C1big_lcg64_2^20x1024", LCG64, 1 << 20, 1024)
+C3_FILL = FillCfg("C3fill_xorwow_2^20x1024", XORWOW, 1 << 20, 1024)
+
+# C5a: L=4, beta=0.3 vs exact enumeration; 8 streams (K = 1 site per stream per colour)
+C5A_PHILOX = IsingCfg("C5a_ising_L4_philox", PHILOX4X32_10, 4, 0.3, 8, 1000)
+C5A_XORWOW = IsingCfg("C5a_ising_L4_xorwow", XORWOW, 4, 0.3, 8, 1000)
+# C5b: L=8192 at beta_c, 1000 sweeps from a random start
+C5B_PHILOX = IsingCfg("C5b_ising_L8192_philox_K4", PHILOX4X32_10, 8192, BETA_C, 1 << 23, 1000)
+C5B_XORWOW = IsingCfg("C5b_ising_L8192_xorwow_K256", XORWOW, 8192, BETA_C, 1 << 17, 1000)
+C5B_XORWOW_K8 = IsingCfg("C5b_ising_L8192_xorwow_K8", XORWOW, 8192, BETA_C, 1 << 22, 1000)
+
+FILL_CONFIGS = [C1, C2, C3_FILL, C1_BIG, C4_FILL]
+DRAW_CONFIGS = [C3, C4_DRAW]
+ISING_CONFIGS = [C5A_PHILOX, C5A_XORWOW, C5B_PHILOX, C5B_XORWOW, C5B_XORWOW_K8]

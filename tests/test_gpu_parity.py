@@ -1,0 +1,303 @@
+"""-m gpu: parity tests proper.  The CUDA path, called through the C-ABI, against the
+CPU oracle, element by element, on the same seeds.  Bar: BIT-EXACT for every integer
+stream, every float conversion (compared as bit patterns), every checksum, every
+generator state and every spin configuration (north_star)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402  (test infrastructure)
+import paper_1204_6193_b200 as pkg  # noqa: E402
+
+KINDS = list(pkg.KIND_NAMES)
+IDS = [pkg.KIND_NAMES[k] for k in KINDS]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _device():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (no CPU fallback exists)")
+    from paper_1204_6193_b200 import build
+    build.build()
+    torch.cuda.set_device(0)
+    yield
+    torch.cuda.synchronize()
+
+
+def dev_u32(n):
+    return torch.empty(max(n, 4), dtype=torch.int32, device="cuda")
+
+
+def host(t, n, dtype=np.uint32):
+    return t.cpu().numpy().view(dtype)[:n]
+
+
+def n_streams_for(kind, S):
+    return S - S % 32 if kind == pkg.RNG_XS1024W else S
+
+
+# ---------------------------------------------------------------------------------
+# fill: several warp tiles + ragged tail in both directions (S not a multiple of 32 /
+# of the CTA size, n not a multiple of 4 / of the 32-draw tile), continuation.
+# ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("S,ns", [(1000, (100, 37, 4, 1, 0, 64)), (33, (3, 129)), (1, (17, 16)), (4096 + 40, (32,))])
+def test_fill_u32_and_continuation(kind, S, ns):
+    S = n_streams_for(kind, S)
+    if S == 0:
+        S = 32
+    g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
+    for n in ns:
+        out = dev_u32(S * n)
+        g.fill_u32(out, n)
+        exp = o.fill_u32(n)
+        got = host(out, S * n)
+        assert np.array_equal(got, exp), f"{pkg.KIND_NAMES[kind]} S={S} n={n}: first diff at {np.flatnonzero(got != exp)[:5]}"
+        assert g.draws_done == o.draws_done
+    if g.state_bytes():
+        assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+def test_fill_f32_bit_patterns(kind):
+    S = n_streams_for(kind, 777)
+    g, o = pkg.Rng(kind, S, 12345), oracle.Rng(kind, S, 12345)
+    for n in (64, 13):
+        out = torch.empty(S * n, dtype=torch.float32, device="cuda")
+        g.fill_f32(out, n)
+        exp = o.fill_f32(n)
+        got = out.cpu().numpy()
+        assert np.array_equal(got.view(np.uint32), exp.view(np.uint32))
+        assert got.min() >= 0.0 and got.max() <= 1.0 - 2.0 ** -24
+    g.close()
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+def test_mixed_call_sequence_is_one_stream(kind):
+    """fill_u32(n1), draw_reduce(n2), fill_f32(n3) continue the same streams (state
+    persists in the handle): compare against one oracle fill of n1+n2+n3."""
+    S = n_streams_for(kind, 300)
+    n1, n2, n3 = 7, 50, 9
+    g, o = pkg.Rng(kind, S, 99), oracle.Rng(kind, S, 99)
+    ref = o.fill_u32(n1 + n2 + n3).reshape(S, -1)
+    a = dev_u32(S * n1)
+    g.fill_u32(a, n1)
+    r = dev_u32(2 * S)
+    g.draw_reduce(r, n2)
+    f = torch.empty(S * n3, dtype=torch.float32, device="cuda")
+    g.fill_f32(f, n3)
+    assert np.array_equal(host(a, S * n1).reshape(S, n1), ref[:, :n1])
+    mid = ref[:, n1:n1 + n2]
+    red = host(r, 2 * S).reshape(S, 2)
+    assert np.array_equal(red[:, 0], np.bitwise_xor.reduce(mid, axis=1))
+    assert np.array_equal(red[:, 1], mid.sum(axis=1, dtype=np.uint64).astype(np.uint32))
+    expf = (ref[:, n1 + n2:] >> 8).astype(np.float32) * np.float32(2.0 ** -24)
+    assert np.array_equal(f.cpu().numpy().reshape(S, n3), expf)
+    g.close()
+
+
+# ---------------------------------------------------------------------------------
+# draw_reduce
+# ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("S,ns", [(2048 + 96, (256, 1, 0, 3, 1001)), (32, (5,))])
+def test_draw_reduce(kind, S, ns):
+    g, o = pkg.Rng(kind, S, 7), oracle.Rng(kind, S, 7)
+    for n in ns:
+        out = dev_u32(2 * S)
+        g.draw_reduce(out, n)
+        assert np.array_equal(host(out, 2 * S), o.draw_reduce(n)), (pkg.KIND_NAMES[kind], S, n)
+    if g.state_bytes():
+        assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
+
+
+# ---------------------------------------------------------------------------------
+# seeding / sharding: a shard [first, first+n_local) of n_total reproduces those rows
+# ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+def test_shard_equals_rows_of_the_whole(kind):
+    n_total, first, n_local, n = 640, 256, 160, 20
+    whole = oracle.Rng(kind, n_total, 3).fill_u32(n).reshape(n_total, n)
+    g = pkg.Rng(kind, n_local, 3, first=first, n_total=n_total)
+    if g.state_bytes():
+        o = oracle.Rng(kind, n_local, 3, first=first, n_total=n_total)
+        assert np.array_equal(g.get_state(), o.get_state()), "seed kernel state != oracle seeding"
+    out = dev_u32(n_local * n)
+    g.fill_u32(out, n)
+    assert np.array_equal(host(out, n_local * n).reshape(n_local, n), whole[first:first + n_local])
+    g.close()
+
+
+def test_lcg_leapfrog_is_one_global_sequence():
+    """all streams generate numbers out of the same global sequence (1)."""
+    S, n = 96, 50
+    g = pkg.Rng(pkg.RNG_LCG64_LEAPFROG, S, 1)
+    out = dev_u32(S * n)
+    g.fill_u32(out, n)
+    got = host(out, S * n).reshape(S, n)
+    x = oracle.splitmix64(1, 0)
+    seq = []
+    for _ in range(S * n):
+        seq.append(x >> 32)
+        x = oracle.lcg64_step(x)
+    assert np.array_equal(got.T.reshape(-1), np.array(seq, dtype=np.uint32))
+    g.close()
+
+
+def test_set_state_roundtrip_and_hand_traced_states():
+    """rng_set_state with the hand-traceable states of tests/golden: XORWOW from
+    (1,0,0,0,0,0) gives 0x587c8 first (R-B1); xs1024 from X0 = 1 (word 31) gives lane
+    31 = 0x587c1, lane 0 = 0x587c0 (R-D5/D6)."""
+    g = pkg.Rng(pkg.RNG_XORWOW, 2, 1)
+    st = np.array([1, 0, 0, 0, 0, 0, 123456789, 362436069, 521288629, 88675123, 5783321, 6615241], dtype=np.uint32)
+    g.set_state(st)
+    assert np.array_equal(g.get_state(), st)
+    out = dev_u32(2 * 8)
+    g.fill_u32(out, 8)
+    got = host(out, 16).reshape(2, 8)
+    assert list(got[0]) == [0x587c8, 0xb0fbd, 0x109a52, 0x165247, 0x1ea6dc, 0x542ed4, 0x329b97a, 0x335f744a]
+    assert list(got[1][:5]) == [246875399, 3690007200, 1264581005, 3906711041, 1866187943]
+    g.close()
+    g = pkg.Rng(pkg.RNG_XS1024W, 32, 1)
+    X = np.zeros(32, dtype=np.uint32)
+    X[31] = 1
+    g.set_state(X)
+    out = dev_u32(32 * 2)
+    g.fill_u32(out, 2)
+    got = host(out, 64).reshape(32, 2)
+    assert got[31, 0] == 0x587c1 and got[0, 0] == 0x587c0
+    assert got[31, 1] == 0xb0f82 and got[0, 1] == 0xb1001
+    g.close()
+
+
+# ---------------------------------------------------------------------------------
+# error behaviour on a live handle
+# ---------------------------------------------------------------------------------
+def test_argument_errors_on_a_live_handle():
+    g = pkg.Rng(pkg.RNG_PHILOX4X32_10, 64, 1)
+    buf = dev_u32(64 * 8 + 4)
+    with pytest.raises(pkg.RngError) as e:
+        pkg.rng_fill_u32(g.handle, buf.data_ptr() + 4, 8)  # misaligned
+    assert e.value.code == pkg.RNG_E_INVAL
+    with pytest.raises(pkg.RngError) as e:
+        pkg.rng_fill_u32(g.handle, None, 8)
+    assert e.value.code == pkg.RNG_E_INVAL
+    sp = torch.zeros(36, dtype=torch.int8, device="cuda")
+    with pytest.raises(pkg.RngError):  # 64 streams do not divide 6*6/2
+        g.ising_sweep(sp, 6, 0.3, 1)
+    with pytest.raises(pkg.RngError):  # odd L
+        g.ising_sweep(sp, 5, 0.3, 1)
+    assert g.draws_done == 0
+    g.close()
+
+
+# ---------------------------------------------------------------------------------
+# Ising consumer
+# ---------------------------------------------------------------------------------
+def test_ising_init_and_energy():
+    for L in (4, 6, 64, 130):
+        sp = torch.empty(L * L + 16, dtype=torch.int8, device="cuda")
+        pkg.ising_init_random(sp, L, 2)
+        ref = oracle.ising_init_random(L, 2)
+        assert np.array_equal(sp.cpu().numpy()[:L * L], ref)
+        e = torch.zeros(1, dtype=torch.int64, device="cuda")
+        pkg.ising_energy(sp, L, e)
+        assert int(e.item()) == oracle.ising_energy(ref, L)
+
+
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("L,S,sweeps", [(4, 8, 50), (4, 1, 20), (6, 6, 10), (64, 256, 12), (64, 2048, 6),
+                                        (128, 32, 4), (256, 4096, 5)])
+def test_ising_sweep_bit_exact(kind, L, S, sweeps):
+    if kind == pkg.RNG_XS1024W and S % 32:
+        pytest.skip("xs1024 needs whole 32-stream instances")
+    beta = 0.3 if L == 4 else 0.44068679350977147
+    g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, 2)
+    ref = oracle.ising_init_random(L, 2)
+    tr = torch.empty(sweeps, dtype=torch.int64, device="cuda")
+    g.ising_sweep(sp, L, beta, sweeps, tr)
+    tr_o = o.ising_sweep(ref, L, beta, sweeps, trace=True)
+    assert np.array_equal(sp.cpu().numpy(), ref), f"lattice differs at {np.flatnonzero(sp.cpu().numpy() != ref)[:8]}"
+    assert np.array_equal(tr.cpu().numpy(), tr_o)
+    assert g.draws_done == o.draws_done == sweeps * L * L // S
+    # a second call continues both the lattice and the streams
+    g.ising_sweep(sp, L, beta, 3)
+    o.ising_sweep(ref, L, beta, 3)
+    assert np.array_equal(sp.cpu().numpy(), ref)
+    if g.state_bytes():
+        assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
+
+
+def test_ising_equals_fill_then_apply():
+    """ising_sweep consumes exactly the draws rng_fill_u32 would have produced
+    (include/rng_b200.h: 'fill K draws per stream, then apply')."""
+    L, S = 32, 64
+    K = L * L // 2 // S
+    g1, g2 = pkg.Rng(pkg.RNG_XORWOW, S, 5), pkg.Rng(pkg.RNG_XORWOW, S, 5)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, 9)
+    g1.ising_sweep(sp, L, 0.4, 2)
+    buf = dev_u32(S * 4 * K)
+    g2.fill_u32(buf, 4 * K)
+    assert np.array_equal(g1.get_state(), g2.get_state())
+    g1.close()
+    g2.close()
+
+
+@pytest.mark.slow
+def test_ising_L4_monte_carlo_energy_within_3_sigma(golden):
+    """C5a: L=4, beta=0.3; <E>/N from the GPU trajectory agrees with the exact
+    enumeration of all 2^16 states (tests/golden/ising_L4.txt) within 3 sigma
+    (binning error), for Philox and XORWOW."""
+    exact = float(golden("ising_L4.txt")["e"][0])
+    L, S, therm, sweeps = 4, 8, 1000, 200000
+    for kind in (pkg.RNG_PHILOX4X32_10, pkg.RNG_XORWOW):
+        g = pkg.Rng(kind, S, 1)
+        sp = torch.empty(16, dtype=torch.int8, device="cuda")
+        pkg.ising_init_random(sp, L, 2)
+        g.ising_sweep(sp, L, 0.3, therm)
+        tr = torch.empty(sweeps, dtype=torch.int64, device="cuda")
+        g.ising_sweep(sp, L, 0.3, sweeps, tr)
+        e = tr.cpu().numpy().astype(np.float64) / 16.0
+        nb = 100
+        bins = e[: (len(e) // nb) * nb].reshape(nb, -1).mean(axis=1)
+        sigma = bins.std(ddof=1) / np.sqrt(nb)
+        assert abs(e.mean() - exact) < 3 * sigma, (pkg.KIND_NAMES[kind], e.mean(), exact, sigma)
+        assert sigma < 5e-3
+        g.close()
+
+
+# ---------------------------------------------------------------------------------
+# host-buffer entry points (the e2e path bench.py times)
+# ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+def test_host_entry_points(kind):
+    S, n = 512, 40
+    g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
+    a = np.empty(S * n, dtype=np.uint32)
+    g.fill_u32_host(a, n)
+    assert np.array_equal(a, o.fill_u32(n))
+    f = np.empty(S * n, dtype=np.float32)
+    g.fill_f32_host(f, n)
+    assert np.array_equal(f.view(np.uint32), o.fill_f32(n).view(np.uint32))
+    r = np.empty(2 * S, dtype=np.uint32)
+    g.draw_reduce_host(r, 33)
+    assert np.array_equal(r, o.draw_reduce(33))
+    g.close()
+    L, S = 64, 128
+    g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
+    sp = oracle.ising_init_random(L, 2)
+    ref = sp.copy()
+    tr = np.empty(4, dtype=np.int64)
+    g.ising_sweep_host(sp, L, 0.4, 4, tr)
+    tr_o = o.ising_sweep(ref, L, 0.4, 4, trace=True)
+    assert np.array_equal(sp, ref) and np.array_equal(tr, tr_o)
+    g.close()
