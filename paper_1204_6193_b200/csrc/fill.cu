@@ -61,6 +61,106 @@ __global__ void __launch_bounds__(256) philox_fill_kernel(uint32_t *__restrict__
 }
 
 // ------------------------------------------------------------------------------------
+// Philox warp-tile fill (the aligned fast path: d0 % 4 == 0 and n % 4 == 0).
+// A tile is 32*U*T consecutive 4-word blocks of ONE row and belongs to one warp; it is
+// processed as T groups of 32*U blocks, lane l computing blocks l, l+32, ... of the group so
+// that every store instruction of the warp writes 512 contiguous bytes.
+//  * The row (hence the key) is fixed per tile and the warp index comes from a broadcast
+//    shuffle, which makes it provably warp-uniform: the ten round keys k + r*(W0,W1) are
+//    computed once per tile in UNIFORM registers and cost no per-thread registers or
+//    per-block instructions.  What is left per round and block is Philox's own arithmetic
+//    (PAPER.md:290-294): 2 IMAD.WIDE + 2 LOP3 (three-input xor with a uniform operand).
+//  * The counter is (lo32(b), hi32(b), 0, 0) (R-C2), so the first round's second S-box
+//    multiplies zero and folds away at compile time.
+//  * U independent blocks per lane are interleaved (the full-tile path has no per-block
+//    predicate, so ptxas keeps them interleaved) and hide the IMAD -> LOP3 -> IMAD chain.
+//  * Persistent grid: warps stride over tiles; (row, tile-in-row) advance incrementally
+//    (one 64-bit division per warp).
+// ------------------------------------------------------------------------------------
+// U independent 4-word blocks per lane (blocks rb0, rb0+32, ...), ten rounds interleaved,
+// one 128-bit streaming store each.  CHECK = bounds-check each block (ragged last tile).
+template <bool F32, int U, bool CHECK>
+__device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_t b0, uint32_t rb0,
+                                             uint32_t blocks_per_row, const uint32_t (&rk0)[10],
+                                             const uint32_t (&rk1)[10])
+{
+    uint32_t c0[U], c1[U], c2[U], c3[U];
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const uint64_t b = b0 + rb0 + 32u * u; // counter = index of the 4-word block (R-C2)
+        c0[u] = (uint32_t)b;
+        c1[u] = (uint32_t)(b >> 32);
+        c2[u] = 0u;
+        c3[u] = 0u;
+    }
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const uint64_t p0 = (uint64_t)kPhM0 * c0[u];
+            const uint64_t p1 = (uint64_t)kPhM1 * c2[u];
+            const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1[u] ^ rk0[r];
+            const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3[u] ^ rk1[r];
+            c1[u] = (uint32_t)p1;
+            c3[u] = (uint32_t)p0;
+            c0[u] = n0;
+            c2[u] = n2;
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const uint32_t rb = rb0 + 32u * u;
+        if (!CHECK || rb < blocks_per_row) {
+            const uint4 v = make_uint4(out_word(c0[u], F32), out_word(c1[u], F32), out_word(c2[u], F32),
+                                       out_word(c3[u], F32));
+            __stcs(reinterpret_cast<uint4 *>(row + 4ull * rb), v); // streaming 128-bit store
+        }
+    }
+}
+
+template <bool F32, int U, int T>
+__global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restrict__ out, uint64_t first, uint64_t seed,
+                                                              uint64_t b0, uint64_t n, uint32_t blocks_per_row,
+                                                              uint32_t tiles_per_row, uint64_t n_tiles)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t warp_in_cta = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0); // warp-uniform by construction
+    const uint64_t n_warps = (uint64_t)gridDim.x * (blockDim.x >> 5);
+    uint64_t t = (uint64_t)blockIdx.x * (blockDim.x >> 5) + warp_in_cta;
+    if (t >= n_tiles) return;
+    uint64_t s = t / tiles_per_row;                    // row of this warp's first tile
+    uint32_t c = (uint32_t)(t - s * tiles_per_row);    // tile within the row
+    const uint64_t ds = n_warps / tiles_per_row;       // per-iteration advance of (s, c)
+    const uint32_t dc = (uint32_t)(n_warps - ds * tiles_per_row);
+    for (; t < n_tiles; t += n_warps) {
+        const uint64_t key = (first + s) ^ seed; // R-C2: key = stream id ^ seed
+        uint32_t rk0[10], rk1[10];
+#pragma unroll
+        for (int r = 0; r < 10; r++) {
+            rk0[r] = (uint32_t)key + (uint32_t)r * kPhW0;
+            rk1[r] = (uint32_t)(key >> 32) + (uint32_t)r * kPhW1;
+        }
+        uint32_t *row = out + s * n;
+        const bool tile_full = (uint64_t)(c + 1u) * (T * 32u * U) <= (uint64_t)blocks_per_row; // warp-uniform
+        if (tile_full) {
+#pragma unroll 1
+            for (int g = 0; g < T; g++)
+                philox_group<F32, U, false>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
+        } else {
+#pragma unroll 1
+            for (int g = 0; g < T; g++)
+                philox_group<F32, U, true>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
+        }
+        s += ds;
+        c += dc;
+        if (c >= tiles_per_row) {
+            c -= tiles_per_row;
+            s++;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------
 // Row-tile fill for stateful generators: thread s owns stream s and its output row.
 // ------------------------------------------------------------------------------------
 constexpr int KT = 32;            // draws per row per tile (one 128-byte line)
@@ -125,6 +225,18 @@ __global__ void __launch_bounds__(FILL_WARPS * 32) rowtile_fill_kernel(Gen g, ui
     if (live) gen.store(g, s);
 }
 
+static int g_sm_count = 0;
+static int sm_count()
+{
+    if (!g_sm_count) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev);
+        if (g_sm_count <= 0) g_sm_count = 148;
+    }
+    return g_sm_count;
+}
+
 template <int KIND>
 static cudaError_t launch_rowtile(const Gen &g, void *d_out, uint64_t n, bool f32, cudaStream_t st)
 {
@@ -139,42 +251,57 @@ static cudaError_t launch_rowtile(const Gen &g, void *d_out, uint64_t n, bool f3
     return cudaGetLastError();
 }
 
-static int g_sm_count = 0;
-static int sm_count()
+template <bool F32, int U, int T>
+static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uint64_t blocks_per_row, cudaStream_t st)
 {
-    if (!g_sm_count) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev);
-        if (g_sm_count <= 0) g_sm_count = 148;
+    const uint64_t tpr = (blocks_per_row + 32 * U * T - 1) / (32 * U * T);
+    const uint64_t n_tiles = g.S * tpr;
+    // persistent grid: a multiple of the SM count; 8 warps per CTA, CTAs resident per SM by registers
+    static int per_sm = 0;
+    if (!per_sm) {
+        int b = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, philox_fill_warp_kernel<F32, U, T>, 256, 0);
+        if (e != cudaSuccess) return e;
+        per_sm = b > 0 ? b : 1;
     }
-    return g_sm_count;
+    uint64_t grid = (uint64_t)sm_count() * per_sm;
+    const uint64_t need = (n_tiles + 7) / 8;
+    if (grid > need) grid = need;
+    philox_fill_warp_kernel<F32, U, T><<<(unsigned)grid, 256, 0, st>>>(o, g.first, g.seed, g.draws_done >> 2, n,
+                                                                     (uint32_t)blocks_per_row, (uint32_t)tpr, n_tiles);
+    count_launch();
+    return cudaGetLastError();
 }
 
-static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, bool f32, cudaStream_t st)
+static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, bool f32, int variant, cudaStream_t st)
 {
-    constexpr int U = 4;
     const uint64_t d0 = g.draws_done;
     const uint64_t blocks_per_row = ((d0 + n - 1) >> 2) - (d0 >> 2) + 1;
+    const bool aligned = ((d0 | n) & 3ull) == 0ull;
+    uint32_t *o = (uint32_t *)d_out;
+    if (aligned && blocks_per_row <= 0x7fffffffull) {
+#define PW(U, T) (f32 ? launch_philox_warp<true, U, T>(g, o, n, blocks_per_row, st) \
+                      : launch_philox_warp<false, U, T>(g, o, n, blocks_per_row, st))
+        switch (variant) { // identical bits; (U, T) = blocks interleaved per lane, groups per tile
+        case 1: return PW(4, 2);
+        case 2: return PW(2, 4);
+        default: return PW(8, 1);
+        }
+#undef PW
+    }
+    // general path: any draw offset / any n, word-by-word stores with bounds checks
+    constexpr int U = 4;
     const uint64_t tpr = (blocks_per_row + 256 * U - 1) / (256 * U);
     if (tpr > 0xffffffffull) return cudaErrorInvalidConfiguration;
     const uint64_t n_tiles = g.S * tpr;
-    const bool aligned = ((d0 | n) & 3ull) == 0ull;
-    // persistent-style grid: a multiple of the SM count, 8 resident CTAs of 256 threads per SM
     uint64_t grid = (uint64_t)sm_count() * 8ull;
     if (grid > n_tiles) grid = n_tiles;
-    uint32_t *o = (uint32_t *)d_out;
-#define PHILOX_LAUNCH(F, A) \
-    philox_fill_kernel<F, A, U><<<(unsigned)grid, 256, 0, st>>>(o, g.S, g.first, g.seed, d0, n, blocks_per_row, \
-                                                              (uint32_t)tpr, n_tiles)
-    if (f32) {
-        if (aligned) PHILOX_LAUNCH(true, true);
-        else PHILOX_LAUNCH(true, false);
-    } else {
-        if (aligned) PHILOX_LAUNCH(false, true);
-        else PHILOX_LAUNCH(false, false);
-    }
-#undef PHILOX_LAUNCH
+    if (f32)
+        philox_fill_kernel<true, false, U><<<(unsigned)grid, 256, 0, st>>>(o, g.S, g.first, g.seed, d0, n, blocks_per_row,
+                                                                          (uint32_t)tpr, n_tiles);
+    else
+        philox_fill_kernel<false, false, U><<<(unsigned)grid, 256, 0, st>>>(o, g.S, g.first, g.seed, d0, n, blocks_per_row,
+                                                                           (uint32_t)tpr, n_tiles);
     count_launch();
     return cudaGetLastError();
 }
@@ -187,7 +314,7 @@ cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, 
     case RNG_LCG64_LEAPFROG: return launch_rowtile<RNG_LCG64_LEAPFROG>(g, d_out, n, f32, st);
     case RNG_XORWOW: return launch_rowtile<RNG_XORWOW>(g, d_out, n, f32, st);
     case RNG_XS1024W: return launch_rowtile<RNG_XS1024W>(g, d_out, n, f32, st);
-    case RNG_PHILOX4X32_10: return launch_philox_fill(g, d_out, n, f32, st);
+    case RNG_PHILOX4X32_10: return launch_philox_fill(g, d_out, n, f32, h.var_store, st);
     default: return cudaErrorInvalidValue;
     }
 }
