@@ -132,6 +132,7 @@ int rng_destroy(rng_handle *h)
     if (h->g.lcg) cudaFree((void *)h->g.lcg);
     if (h->staging) cudaFree(h->staging);
     if (h->energy_scratch) cudaFree(h->energy_scratch);
+    if (h->ms_planes) cudaFree(h->ms_planes);
     delete h;
     return RNG_OK;
 }
@@ -199,6 +200,32 @@ int ising_sweep(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_
     ising_accept_table(beta, nullptr, tab.T);
     cudaStream_t st = (cudaStream_t)stream;
     uint64_t d = h->g.draws_done;
+    if (n_sweeps == 0) return RNG_OK;
+    // variant "ising": 0 = automatic (multi-spin bit planes when the geometry allows and the pack/unpack
+    // pays off, else the byte kernels), 1 = generic byte kernel only, 2 = byte kernels only, 3 = multi-spin
+    // whenever eligible.  Every variant produces the same trajectory.
+    const bool want_ms = h->var_ising == 3 || (h->var_ising == 0 && n_sweeps >= 2);
+    if (want_ms && ising_ms_eligible(*h, L, tab, K, d)) {
+        const uint64_t need = (uint64_t)L * L / 8; // two planes of L*L/64 words
+        if (h->ms_planes_bytes < need) {
+            if (h->ms_planes) cudaFree(h->ms_planes);
+            h->ms_planes = nullptr;
+            h->ms_planes_bytes = 0;
+            CU(cudaMalloc((void **)&h->ms_planes, need));
+            h->ms_planes_bytes = need;
+        }
+        CU(launch_ising_ms_pack(d_spins, h->ms_planes, L, st));
+        for (uint32_t t = 0; t < n_sweeps; t++) {
+            for (int c = 0; c < 2; c++) {
+                CU(launch_ising_ms_half_sweep(*h, h->ms_planes, L, tab, K, d, c, st));
+                d += K;
+            }
+            if (d_trace) CU(launch_ising_ms_energy(h->ms_planes, L, d_trace + t, st));
+        }
+        CU(launch_ising_ms_unpack(d_spins, h->ms_planes, L, st));
+        h->g.draws_done = d;
+        return RNG_OK;
+    }
     for (uint32_t t = 0; t < n_sweeps; t++) {
         for (int c = 0; c < 2; c++) {
             CU(launch_ising_half_sweep(*h, d_spins, L, tab, K, d, c, st));

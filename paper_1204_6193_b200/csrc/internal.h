@@ -43,6 +43,8 @@ struct rng_handle {
     void *staging;          // device staging for the *_host entry points
     uint64_t staging_bytes;
     int64_t *energy_scratch; // device, 1 x int64
+    uint32_t *ms_planes;     // device scratch of the multi-spin Ising path: two bit planes of L*L/64 words
+    uint64_t ms_planes_bytes;
     int var_xs1024, var_ising, var_store;
 };
 
@@ -62,6 +64,13 @@ struct IsingTable {
 };
 cudaError_t launch_ising_half_sweep(const rng_handle &h, int8_t *d_spins, uint32_t L, const IsingTable &tab,
                                     uint64_t K, uint64_t draws_done, int colour, cudaStream_t st);
+// ising_ms.cu (multi-spin-coded half-sweeps on bit planes; same trajectory as ising.cu)
+bool ising_ms_eligible(const rng_handle &h, uint32_t L, const IsingTable &tab, uint64_t K, uint64_t draws_done);
+cudaError_t launch_ising_ms_pack(const int8_t *d_spins, uint32_t *planes, uint32_t L, cudaStream_t st);
+cudaError_t launch_ising_ms_unpack(int8_t *d_spins, const uint32_t *planes, uint32_t L, cudaStream_t st);
+cudaError_t launch_ising_ms_energy(const uint32_t *planes, uint32_t L, int64_t *d_out, cudaStream_t st);
+cudaError_t launch_ising_ms_half_sweep(const rng_handle &h, uint32_t *planes, uint32_t L, const IsingTable &tab, uint64_t K,
+                                       uint64_t draws_done, int colour, cudaStream_t st);
 cudaError_t launch_ising_init_random(int8_t *d_spins, uint32_t L, uint64_t seed, cudaStream_t st);
 cudaError_t launch_ising_energy(const int8_t *d_spins, uint32_t L, int64_t *d_out, cudaStream_t st);
 

@@ -1,0 +1,358 @@
+// ising_ms.cu -- a8, multi-spin-coded form of the checkerboard Metropolis half-sweep
+// (BASELINE.json config 5; readings R-E1..E7).  Same trajectory, bit for
+// bit, as the byte kernels in ising.cu: only the in-flight representation differs.
+//
+// Representation (device scratch owned by the handle, alive for one ising_sweep call):
+// one bit plane per colour, plane_c[q >> 5] bit (q & 31) = 1 iff the spin of the colour-c
+// site q is -1, with q = y*(L/2) + xh the site number of R-E6 (x = 2*xh + ((y+c)&1)).
+// A 32-bit word is 32 consecutive sites of one row (needs L % 64 == 0).  The int8 lattice
+// is packed once at the start of ising_sweep and unpacked once at the end.
+//
+// Neighbours of the 32 sites of word (y, j) of colour c, all in the OTHER plane N:
+//   up    N[(y-1) W + j]      down  N[(y+1) W + j]      same index  N[y W + j]
+//   and the same row shifted by one site: towards xh-1 if p = (y+c)&1 is 0, towards xh+1
+//   if p is 1 (one funnel shift with the adjacent word, periodic).
+// nbar = number of neighbours anti-aligned with the site = bit-sliced sum of the four
+// words (N_k xor C); aligned neighbours (h+4)/2 = 4 - nbar.  For beta >= 0 the Metropolis
+// table has T[i] = 2^24 (always flip) for h <= 0, so
+//   flip = (nbar >= 2) | (r <= thr0) | ((nbar & 1) & (r <= thr1)),
+//   thr0 = 256 T[4] - 1 (nbar = 0), thr1 = 256 T[3] - 1 (nbar = 1), thr0 <= thr1,
+// where (r >> 8) < T  <=>  r <= 256 T - 1 for 1 <= T <= 2^24.  The host takes the byte
+// kernels when the table does not have this shape.
+//
+// The two compares of a draw are two carry chains: sub.cc thr - r leaves the carry flag set
+// iff there is no borrow (r <= thr: the hardware subtracts as thr + ~r + 1), and
+// addc acc,acc,acc shifts that flag into an accumulator; after 32 draws the bit-reversed
+// accumulator is the word of accept bits.  4 integer adds per site, no
+// per-site table lookup, select or byte extraction; the random numbers stay in registers.
+//
+// Thread <-> stream mapping (R-E6: stream s owns sites [sK, (s+1)K) and spends one draw
+// per site in increasing q):
+//   STREAM mode (K % 32 == 0): one thread per stream, its K/32 words in order, generator
+//     state in registers for all K draws (the paper's "many numbers per state load"
+//     regime).
+//   WORD mode (K in {4, 8, 16}): one thread per word = 32/K consecutive streams.
+#include "internal.h"
+#include "streams.cuh"
+
+namespace rngb200 {
+
+struct MsThr {
+    uint32_t thr0, thr1;
+};
+
+// acc <- 2 acc + (r <= thr), for both thresholds
+__device__ __forceinline__ void ms_cmp_insert(uint32_t r, const MsThr &t, uint32_t &n0, uint32_t &n1)
+{
+    asm("{\n\t"
+        ".reg .u32 t;\n\t"
+        "sub.cc.u32 t, %2, %4;\n\t"
+        "addc.u32 %0, %0, %0;\n\t"
+        "sub.cc.u32 t, %3, %4;\n\t"
+        "addc.u32 %1, %1, %1;\n\t"
+        "}"
+        : "+r"(n0), "+r"(n1)
+        : "r"(t.thr0), "r"(t.thr1), "r"(r));
+}
+
+// the four neighbour words of word (y, j) and the word itself
+struct MsWord {
+    uint32_t *cptr;
+    uint32_t C, U, D, H0, H1;
+    __device__ __forceinline__ void load(uint32_t *__restrict__ Cp, const uint32_t *__restrict__ Np, uint32_t L,
+                                         uint32_t wpr, uint32_t y, uint32_t j, uint32_t colour)
+    {
+        const uint32_t yu = y ? y - 1u : L - 1u, yd = (y + 1u == L) ? 0u : y + 1u;
+        const uint32_t base = y * wpr;
+        cptr = Cp + base + j;
+        C = *cptr;
+        U = Np[yu * wpr + j];
+        D = Np[yd * wpr + j];
+        H0 = Np[base + j];
+        if (((y + colour) & 1u) == 0u) { // active sites at even x: other horizontal neighbour is xh-1
+            const uint32_t Hn = Np[base + (j ? j - 1u : wpr - 1u)];
+            H1 = __funnelshift_l(Hn, H0, 1); // (H0 << 1) | (Hn >> 31)
+        } else {
+            const uint32_t Hn = Np[base + (j + 1u == wpr ? 0u : j + 1u)];
+            H1 = __funnelshift_r(H0, Hn, 1); // (H0 >> 1) | (Hn << 31)
+        }
+    }
+    // n0, n1: bit (31-k) = (r_k <= thr0 / thr1), k = site within the word
+    __device__ __forceinline__ void update_store(uint32_t n0, uint32_t n1)
+    {
+        const uint32_t A0 = __brev(n0), A1 = __brev(n1);
+        const uint32_t x0 = U ^ C, x1 = D ^ C, x2 = H0 ^ C, x3 = H1 ^ C;
+        const uint32_t s = x0 ^ x1 ^ x2, cy = (x0 & x1) | (x0 & x2) | (x1 & x2);
+        const uint32_t b0 = s ^ x3, cy2 = s & x3;
+        const uint32_t flip = (cy | cy2) | A0 | (b0 & A1);
+        *cptr = C ^ flip;
+    }
+};
+
+// ---- STREAM mode -------------------------------------------------------------------
+template <int KIND>
+__global__ void __launch_bounds__(64) ising_ms_stream_kernel(Gen g, uint32_t *__restrict__ Cp,
+                                                             const uint32_t *__restrict__ Np, uint32_t L, MsThr thr,
+                                                             uint32_t W, uint32_t colour)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= g.S) return; // xs1024: S % 32 == 0 and blockDim % 32 == 0, whole warps leave together
+    const uint32_t wpr = L >> 6;
+    uint32_t widx = (uint32_t)s * W;
+    uint32_t y = widx / wpr, j = widx - y * wpr;
+    if (KIND == RNG_PHILOX4X32_10) {
+        const uint64_t key = (g.first + s) ^ g.seed;
+        const uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
+        uint64_t b = g.draws_done >> 2; // draws_done % 4 == 0 (host-checked): whole blocks
+        for (uint32_t i = 0; i < W; i++) {
+            MsWord mw;
+            mw.load(Cp, Np, L, wpr, y, j, colour);
+            uint32_t n0 = 0u, n1 = 0u;
+#pragma unroll
+            for (int gi = 0; gi < 8; gi++, b++) {
+                const uint4 o = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+                ms_cmp_insert(o.x, thr, n0, n1);
+                ms_cmp_insert(o.y, thr, n0, n1);
+                ms_cmp_insert(o.z, thr, n0, n1);
+                ms_cmp_insert(o.w, thr, n0, n1);
+            }
+            mw.update_store(n0, n1);
+            if (++j == wpr) {
+                j = 0;
+                y++;
+            }
+        }
+    } else {
+        Stream<KIND> gen;
+        gen.load(g, s);
+        for (uint32_t i = 0; i < W; i++) {
+            MsWord mw;
+            mw.load(Cp, Np, L, wpr, y, j, colour);
+            uint32_t n0 = 0u, n1 = 0u;
+#pragma unroll
+            for (int k = 0; k < 32; k++) ms_cmp_insert(gen.next(), thr, n0, n1);
+            mw.update_store(n0, n1);
+            if (++j == wpr) {
+                j = 0;
+                y++;
+            }
+        }
+        gen.store(g, s);
+    }
+}
+
+// ---- WORD mode: K in {4, 8, 16}, 32/K streams per word -------------------------------
+template <int KIND, int K>
+__global__ void __launch_bounds__(128) ising_ms_word_kernel(Gen g, uint32_t *__restrict__ Cp,
+                                                            const uint32_t *__restrict__ Np, uint32_t L, MsThr thr,
+                                                            uint32_t n_words, uint32_t colour)
+{
+    const uint32_t widx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (widx >= n_words) return;
+    const uint32_t wpr = L >> 6;
+    const uint32_t y = widx / wpr, j = widx - y * wpr;
+    MsWord mw;
+    mw.load(Cp, Np, L, wpr, y, j, colour);
+    uint32_t n0 = 0u, n1 = 0u;
+    const uint64_t s0 = (uint64_t)widx * (32 / K);
+    if (KIND == RNG_PHILOX4X32_10) {
+        const uint64_t b0 = g.draws_done >> 2; // draws_done % 4 == 0
+#pragma unroll
+        for (int gi = 0; gi < 8; gi++) {
+            const uint64_t s = s0 + (4 * gi) / K;
+            const uint64_t b = b0 + ((4 * gi) % K) / 4;
+            const uint64_t key = (g.first + s) ^ g.seed;
+            const uint4 o = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, (uint32_t)key, (uint32_t)(key >> 32));
+            ms_cmp_insert(o.x, thr, n0, n1);
+            ms_cmp_insert(o.y, thr, n0, n1);
+            ms_cmp_insert(o.z, thr, n0, n1);
+            ms_cmp_insert(o.w, thr, n0, n1);
+        }
+    } else {
+#pragma unroll
+        for (int a = 0; a < 32 / K; a++) {
+            Stream<KIND> gen;
+            gen.load(g, s0 + a);
+#pragma unroll
+            for (int k = 0; k < K; k++) ms_cmp_insert(gen.next(), thr, n0, n1);
+            gen.store(g, s0 + a);
+        }
+    }
+    mw.update_store(n0, n1);
+}
+
+// ---- pack / unpack / energy ----------------------------------------------------------
+// thread per 64 bytes of a row: even-x bytes are colour (y&1), odd-x bytes the other one
+__global__ void __launch_bounds__(256) ising_ms_pack_kernel(const int8_t *__restrict__ sp, uint32_t *__restrict__ plane0,
+                                                            uint32_t *__restrict__ plane1, uint32_t L, uint32_t n_words)
+{
+    const uint32_t widx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (widx >= n_words) return;
+    const uint32_t wpr = L >> 6, y = widx / wpr, j = widx - y * wpr;
+    const uint4 *src = reinterpret_cast<const uint4 *>(sp + (uint64_t)y * L + 64u * j);
+    uint32_t e = 0u, o = 0u;
+#pragma unroll
+    for (int v = 0; v < 4; v++) {
+        const uint4 q = src[v];
+        const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+        for (int k = 0; k < 4; k++) {
+            const int kk = 4 * v + k; // word of the 64-byte run: bytes 4kk .. 4kk+3 = sites 2kk, 2kk+1 of each colour
+            e |= ((w[k] >> 1) & 1u) << (2 * kk) | ((w[k] >> 17) & 1u) << (2 * kk + 1); // -1 = 0xff has bit 1 set
+            o |= ((w[k] >> 9) & 1u) << (2 * kk) | ((w[k] >> 25) & 1u) << (2 * kk + 1);
+        }
+    }
+    if (y & 1u) {
+        plane1[widx] = e;
+        plane0[widx] = o;
+    } else {
+        plane0[widx] = e;
+        plane1[widx] = o;
+    }
+}
+
+__global__ void __launch_bounds__(256) ising_ms_unpack_kernel(int8_t *__restrict__ sp, const uint32_t *__restrict__ plane0,
+                                                              const uint32_t *__restrict__ plane1, uint32_t L,
+                                                              uint32_t n_words)
+{
+    const uint32_t widx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (widx >= n_words) return;
+    const uint32_t wpr = L >> 6, y = widx / wpr, j = widx - y * wpr;
+    const uint32_t e = (y & 1u) ? plane1[widx] : plane0[widx];
+    const uint32_t o = (y & 1u) ? plane0[widx] : plane1[widx];
+    uint4 *dst = reinterpret_cast<uint4 *>(sp + (uint64_t)y * L + 64u * j);
+#pragma unroll
+    for (int v = 0; v < 4; v++) {
+        uint32_t w[4];
+#pragma unroll
+        for (int k = 0; k < 4; k++) {
+            const int kk = 4 * v + k;
+            const uint32_t f = ((e >> (2 * kk)) & 1u) | ((o >> (2 * kk)) & 1u) << 8 | ((e >> (2 * kk + 1)) & 1u) << 16 |
+                               ((o >> (2 * kk + 1)) & 1u) << 24;
+            w[k] = 0x01010101u + f * 0xfeu; // +1 = 0x01, -1 = 0xff
+        }
+        dst[v] = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+}
+
+// E = -sum_<ij> s_i s_j.  Every bond joins the two colours, so summing nbar over the sites
+// of colour 0 counts each anti-aligned bond once:  E = 2 * anti - 2 * L^2.
+__global__ void __launch_bounds__(256) ising_ms_energy_kernel(const uint32_t *__restrict__ plane0,
+                                                              const uint32_t *__restrict__ plane1, uint32_t L,
+                                                              uint32_t n_words, unsigned long long *__restrict__ out)
+{
+    const uint32_t wpr = L >> 6;
+    long long acc = 0;
+    for (uint32_t widx = blockIdx.x * blockDim.x + threadIdx.x; widx < n_words; widx += gridDim.x * blockDim.x) {
+        const uint32_t y = widx / wpr, j = widx - y * wpr;
+        MsWord mw;
+        mw.load(const_cast<uint32_t *>(plane0), plane1, L, wpr, y, j, 0u);
+        const uint32_t x0 = mw.U ^ mw.C, x1 = mw.D ^ mw.C, x2 = mw.H0 ^ mw.C, x3 = mw.H1 ^ mw.C;
+        acc += __popc(x0) + __popc(x1) + __popc(x2) + __popc(x3);
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    __shared__ long long part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long t = 0;
+        for (int w = 0; w < 8; w++) t += part[w];
+        t *= 2;
+        if (blockIdx.x == 0) t -= 2ll * (long long)L * (long long)L;
+        atomicAdd(out, (unsigned long long)t);
+    }
+}
+
+// ---- host side -----------------------------------------------------------------------
+bool ising_ms_eligible(const rng_handle &h, uint32_t L, const IsingTable &tab, uint64_t K, uint64_t draws_done)
+{
+    if (L % 64u || L > 65536u) return false;
+    const uint32_t one = 1u << 24;
+    if (tab.T[0] != one || tab.T[1] != one || tab.T[2] != one) return false;
+    if (tab.T[4] < 1u || tab.T[4] > tab.T[3] || tab.T[3] > one) return false;
+    const int kind = h.g.kind;
+    if (kind == RNG_PHILOX4X32_10 && (draws_done & 3ull)) return false;
+    if (K % 32ull == 0ull) return K / 32ull <= 0xffffffffull && h.g.S <= 0x7fffffffull;
+    if (K == 4 || K == 8 || K == 16) return kind != RNG_XS1024W;
+    return false;
+}
+
+cudaError_t launch_ising_ms_pack(const int8_t *d_spins, uint32_t *planes, uint32_t L, cudaStream_t st)
+{
+    const uint32_t n_words = (uint32_t)((uint64_t)L * L / 64);
+    ising_ms_pack_kernel<<<(n_words + 255) / 256, 256, 0, st>>>(d_spins, planes, planes + n_words, L, n_words);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ising_ms_unpack(int8_t *d_spins, const uint32_t *planes, uint32_t L, cudaStream_t st)
+{
+    const uint32_t n_words = (uint32_t)((uint64_t)L * L / 64);
+    ising_ms_unpack_kernel<<<(n_words + 255) / 256, 256, 0, st>>>(d_spins, planes, planes + n_words, L, n_words);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ising_ms_energy(const uint32_t *planes, uint32_t L, int64_t *d_out, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(d_out, 0, sizeof(int64_t), st);
+    if (e != cudaSuccess) return e;
+    const uint32_t n_words = (uint32_t)((uint64_t)L * L / 64);
+    uint32_t grid = (n_words + 255) / 256;
+    if (grid > 148u * 8u) grid = 148u * 8u;
+    ising_ms_energy_kernel<<<grid, 256, 0, st>>>(planes, planes + n_words, L, n_words, (unsigned long long *)d_out);
+    count_launch();
+    return cudaGetLastError();
+}
+
+template <int KIND>
+static void launch_ms_word(const Gen &g, uint32_t *Cp, const uint32_t *Np, uint32_t L, MsThr thr, uint32_t n_words,
+                           uint64_t K, uint32_t colour, cudaStream_t st)
+{
+    const uint32_t grid = (n_words + 127) / 128;
+    switch (K) {
+    case 4: ising_ms_word_kernel<KIND, 4><<<grid, 128, 0, st>>>(g, Cp, Np, L, thr, n_words, colour); break;
+    case 8: ising_ms_word_kernel<KIND, 8><<<grid, 128, 0, st>>>(g, Cp, Np, L, thr, n_words, colour); break;
+    default: ising_ms_word_kernel<KIND, 16><<<grid, 128, 0, st>>>(g, Cp, Np, L, thr, n_words, colour); break;
+    }
+}
+
+cudaError_t launch_ising_ms_half_sweep(const rng_handle &h, uint32_t *planes, uint32_t L, const IsingTable &tab, uint64_t K,
+                                       uint64_t draws_done, int colour, cudaStream_t st)
+{
+    Gen g = h.g;
+    g.draws_done = draws_done;
+    const uint32_t n_words = (uint32_t)((uint64_t)L * L / 64);
+    uint32_t *Cp = planes + (colour ? n_words : 0u);
+    const uint32_t *Np = planes + (colour ? 0u : n_words);
+    MsThr thr;
+    thr.thr0 = (uint32_t)(((uint64_t)tab.T[4] << 8) - 1ull);
+    thr.thr1 = (uint32_t)(((uint64_t)tab.T[3] << 8) - 1ull);
+    if (K % 32ull == 0ull) {
+        const uint32_t W = (uint32_t)(K / 32ull);
+        const uint32_t grid = (uint32_t)((g.S + 63) / 64);
+#define MS_STREAM(KIND) ising_ms_stream_kernel<KIND><<<grid, 64, 0, st>>>(g, Cp, Np, L, thr, W, (uint32_t)colour)
+        switch (g.kind) {
+        case RNG_LCG64: MS_STREAM(RNG_LCG64); break;
+        case RNG_LCG64_LEAPFROG: MS_STREAM(RNG_LCG64_LEAPFROG); break;
+        case RNG_XORWOW: MS_STREAM(RNG_XORWOW); break;
+        case RNG_XS1024W: MS_STREAM(RNG_XS1024W); break;
+        case RNG_PHILOX4X32_10: MS_STREAM(RNG_PHILOX4X32_10); break;
+        default: return cudaErrorInvalidValue;
+        }
+#undef MS_STREAM
+    } else {
+        switch (g.kind) {
+        case RNG_LCG64: launch_ms_word<RNG_LCG64>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
+        case RNG_LCG64_LEAPFROG: launch_ms_word<RNG_LCG64_LEAPFROG>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
+        case RNG_XORWOW: launch_ms_word<RNG_XORWOW>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
+        case RNG_PHILOX4X32_10: launch_ms_word<RNG_PHILOX4X32_10>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
+        default: return cudaErrorInvalidValue;
+        }
+    }
+    count_launch();
+    return cudaGetLastError();
+}
+
+} // namespace rngb200

@@ -212,7 +212,8 @@ def test_ising_init_and_energy():
 
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 @pytest.mark.parametrize("L,S,sweeps", [(4, 8, 50), (4, 1, 20), (6, 6, 10), (64, 256, 12), (64, 2048, 6),
-                                        (128, 32, 4), (256, 4096, 5)])
+                                        (128, 32, 4), (256, 4096, 5), (512, 16384, 3), (48, 96, 5), (64, 512, 4),
+                                        (1024, 1024, 2)])
 def test_ising_sweep_bit_exact(kind, L, S, sweeps):
     if kind == pkg.RNG_XS1024W and S % 32:
         pytest.skip("xs1024 needs whole 32-stream instances")
@@ -234,6 +235,57 @@ def test_ising_sweep_bit_exact(kind, L, S, sweeps):
     if g.state_bytes():
         assert np.array_equal(g.get_state(), o.get_state())
     g.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2, 3], ids=["auto", "generic", "bytes", "multispin"])
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("L,S,sweeps", [(64, 64, 5), (128, 32, 4), (256, 4096, 4), (64, 512, 4), (128, 512, 3),
+                                        (192, 576, 3), (512, 16384, 2), (1024, 1024, 2)])
+def test_ising_kernel_variants_share_one_trajectory(kind, L, S, sweeps, variant):
+    """every kernel variant (generic byte kernel, 16-byte chunk kernel, multi-spin bit planes in
+    STREAM and WORD mode) reproduces the oracle's lattice, energy trace and generator state"""
+    if kind == pkg.RNG_XS1024W and S % 32:
+        pytest.skip("xs1024 needs whole 32-stream instances")
+    beta = 0.44068679350977147
+    g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
+    g.set_variant("ising", variant)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, 2)
+    ref = oracle.ising_init_random(L, 2)
+    tr = torch.empty(sweeps, dtype=torch.int64, device="cuda")
+    g.ising_sweep(sp, L, beta, sweeps, tr)
+    tr_o = o.ising_sweep(ref, L, beta, sweeps, trace=True)
+    assert np.array_equal(sp.cpu().numpy(), ref), f"lattice differs at {np.flatnonzero(sp.cpu().numpy() != ref)[:8]}"
+    assert np.array_equal(tr.cpu().numpy(), tr_o)
+    # misalign the draw counter (Philox must leave its whole-block fast paths), then continue without a trace
+    red = dev_u32(2 * S)
+    g.draw_reduce(red, 3)
+    o.draw_reduce(3)
+    g.ising_sweep(sp, L, beta, 2)
+    o.ising_sweep(ref, L, beta, 2)
+    assert np.array_equal(sp.cpu().numpy(), ref)
+    assert g.draws_done == o.draws_done
+    if g.state_bytes():
+        assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
+
+
+@pytest.mark.parametrize("beta", [0.0, 0.3, 1.5, 20.0, -0.2])
+def test_ising_variants_at_other_temperatures(beta):
+    """beta = 0 (every move accepted), large beta (thresholds down to T = 0 ... never accepted) and
+    beta < 0 (table shape the fast paths do not cover): all fall back correctly"""
+    L, S, sweeps = 128, 1024, 3
+    for kind in (pkg.RNG_PHILOX4X32_10, pkg.RNG_XORWOW):
+        for variant in (0, 2, 3):
+            g, o = pkg.Rng(kind, S, 7), oracle.Rng(kind, S, 7)
+            g.set_variant("ising", variant)
+            sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+            pkg.ising_init_random(sp, L, 3)
+            ref = oracle.ising_init_random(L, 3)
+            g.ising_sweep(sp, L, beta, sweeps)
+            o.ising_sweep(ref, L, beta, sweeps)
+            assert np.array_equal(sp.cpu().numpy(), ref), (beta, kind, variant)
+            g.close()
 
 
 def test_ising_equals_fill_then_apply():
