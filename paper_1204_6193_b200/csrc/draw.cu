@@ -75,6 +75,7 @@ __global__ void __launch_bounds__(256) philox_draw_reduce_kernel(Gen g, uint2 *_
 cudaError_t launch_draw_reduce(const rng_handle &h, uint32_t *d_out, uint64_t n, cudaStream_t st)
 {
     const Gen &g = h.g;
+    if (g.kind == RNG_XS1024W && h.var_xs1024 != 64) return launch_xs1024_draw(h, d_out, n, st);
     const uint64_t grid = (g.S + 255) / 256;
     if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
     uint2 *o = (uint2 *)d_out;

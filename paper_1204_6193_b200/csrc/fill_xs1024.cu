@@ -1,0 +1,260 @@
+// fill_xs1024.cu -- fill and in-register draw kernels of the paper's XORShift1024/Weyl
+// generator for an instance spread
+// over P = 32/K lanes (xs1024.cuh).  Results are identical for every K; K is a measurement
+// knob (rng_set_variant("xs1024", K)), the default is chosen per mode from B200 measurements
+// (DESIGN.md section 6).
+//
+// Streams 32g..32g+31 are the words of instance g (R-D4), so lane l of a warp that hosts K
+// instances owns the K consecutive rows K*l .. K*l+K-1 of the warp's 32K rows: state loads
+// and stores are one contiguous K-word access per lane.
+//
+// Fill mode writes stream-major rows, so a row only becomes a full 128-byte line after 32
+// updates of its instance.  The warp therefore stages a [32K rows][32 draws] tile in shared
+// memory and writes whole lines (a B200 microbenchmark of the alternative -- each thread
+// storing 32-byte row pieces directly -- reaches only 1.4 TB/s: partially written lines get
+// evicted from L2).  See xs1024_fill_kernel for the tile layout and the TMA bulk-store write-out.
+#include "internal.h"
+#include "xs1024.cuh"
+
+namespace rngb200 {
+
+// ---- TMA bulk store of one staged row (shared -> global), issued by the lane that wrote it ----
+__device__ __forceinline__ void bulk_store_row(uint32_t *gdst, const uint32_t *ssrc, uint32_t bytes)
+{
+    const uint32_t saddr = (uint32_t)__cvta_generic_to_shared(ssrc);
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(saddr), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_fence_generic_to_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
+constexpr int XS_ROW_WORDS = 36; // staged row: 32 draws + 4 words of padding (16-byte aligned, conflict-free)
+
+// Tile layout: row r = K*lane + j of the warp sits in slot j*32 + lane, slots are XS_ROW_WORDS
+// apart: the 128-bit stores of the eight lanes of a quarter-warp hit eight different bank
+// groups, and a staged row is contiguous, as a bulk copy needs.
+// BULK: every lane hands its own K rows to the TMA unit (cp.async.bulk shared -> global, one
+// 128-byte line per copy) and goes on generating; it waits for the copies to have READ the
+// tile only just before it overwrites it.  No warp synchronisation, no LDS/STG write-out.
+// !BULK (and every ragged or unaligned tile): write-out with LDS.128 + streaming STG.128.
+template <int K, bool F32, int WARPS, bool BULK>
+__global__ void __launch_bounds__(WARPS * 32) xs1024_fill_kernel(Gen g, uint32_t *__restrict__ out, uint64_t n)
+{
+    extern __shared__ __align__(16) uint32_t xs_tiles[];
+    constexpr int P = 32 / K;
+    constexpr int ROWS = 32 * K;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *tile = xs_tiles + warp * (ROWS * XS_ROW_WORDS);
+    const uint64_t s0 = ((uint64_t)blockIdx.x * WARPS + warp) * (uint64_t)ROWS; // first row of this warp
+    if (s0 >= g.S) return;                                                      // warp-uniform
+    const int p = (P == 1) ? 0 : (lane & (P - 1));
+    const uint64_t my0 = s0 + (uint64_t)K * lane; // S % 32 == 0 and K | 32: my K rows are all live or all dead
+    const bool live = my0 < g.S;
+    const uint32_t rows = (uint32_t)((g.S - s0 < (uint64_t)ROWS) ? (g.S - s0) : (uint64_t)ROWS);
+    const bool vec_ok = (n & 3ull) == 0ull;
+    uint32_t *state = (uint32_t *)g.state;
+
+    uint32_t w[K];
+#pragma unroll
+    for (int j = 0; j < K; j++) w[j] = 0u;
+    if (live) load_words<K>(state + my0, w);
+    XsMasks<K> m;
+    m.init(p);
+    uint32_t nupd = (uint32_t)g.draws_done; // the Weyl term only needs the update count mod 2^32
+    uint32_t *myrows = tile + lane * XS_ROW_WORDS; // + j * 32 * XS_ROW_WORDS
+    uint32_t *grow = out + my0 * n;                // my first row in the output
+    bool pending = false;                          // bulk copies of mine may still be reading the tile
+
+    for (uint64_t j0 = 0; j0 < n; j0 += 32) {
+        const uint32_t kk = (uint32_t)((n - j0 < 32ull) ? (n - j0) : 32ull);
+        // ---- generate kk updates; lane writes draws of its K rows, four at a time ----
+        uint32_t c = 0;
+        for (; 4u * c + 4u <= kk; c++) {
+            uint32_t o[K][4];
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                xs1024_update_k<K>(w, m);
+                nupd++;
+                const uint32_t wt = xs1024_weyl_term(nupd);
+#pragma unroll
+                for (int j = 0; j < K; j++) o[j][u] = out_word(wt + w[j], F32);
+            }
+            if (BULK && pending) {
+                bulk_wait_read_all();
+                pending = false;
+            }
+#pragma unroll
+            for (int j = 0; j < K; j++)
+                *reinterpret_cast<uint4 *>(myrows + j * (32 * XS_ROW_WORDS) + 4u * c) =
+                    make_uint4(o[j][0], o[j][1], o[j][2], o[j][3]);
+        }
+        if (4u * c < kk) { // ragged tail of the call
+            if (BULK && pending) {
+                bulk_wait_read_all();
+                pending = false;
+            }
+            for (uint32_t u = 4u * c; u < kk; u++) {
+                xs1024_update_k<K>(w, m);
+                nupd++;
+                const uint32_t wt = xs1024_weyl_term(nupd);
+#pragma unroll
+                for (int j = 0; j < K; j++) myrows[j * (32 * XS_ROW_WORDS) + u] = out_word(wt + w[j], F32);
+            }
+        }
+        if (BULK && kk == 32u && vec_ok) {
+            // ---- hand my K rows to the TMA unit: 128 contiguous bytes each ----
+            if (live) {
+                bulk_fence_generic_to_async();
+#pragma unroll
+                for (int j = 0; j < K; j++) bulk_store_row(grow + (uint64_t)j * n + j0, myrows + j * (32 * XS_ROW_WORDS), 128u);
+                bulk_commit();
+                pending = true;
+            }
+            continue;
+        }
+        __syncwarp();
+        // ---- write out: every warp instruction stores four complete 128-byte lines ----
+        if (kk == 32u && vec_ok) {
+            // lane -> chunk (lane & 7) of rows (lane >> 3), +4, +8, ...
+            const uint32_t ch = (uint32_t)lane & 7u, r0 = (uint32_t)lane >> 3;
+            uint32_t *gp = out + (s0 + r0) * n + j0 + 4u * ch;
+            const uint64_t gstep = 4ull * n;
+            if (rows == (uint32_t)ROWS) {
+#pragma unroll 8
+                for (int it = 0; it < 8 * K; it++) {
+                    const uint32_t r = 4u * (uint32_t)it + r0;
+                    const uint32_t slot = (r % K) * 32u + r / K;
+                    const uint4 v = *reinterpret_cast<const uint4 *>(tile + slot * XS_ROW_WORDS + 4u * ch);
+                    __stcs(reinterpret_cast<uint4 *>(gp), v);
+                    gp += gstep;
+                }
+            } else {
+                for (uint32_t r = r0; r < rows; r += 4u, gp += gstep) {
+                    const uint32_t slot = (r % K) * 32u + r / K;
+                    const uint4 v = *reinterpret_cast<const uint4 *>(tile + slot * XS_ROW_WORDS + 4u * ch);
+                    __stcs(reinterpret_cast<uint4 *>(gp), v);
+                }
+            }
+        } else {
+            for (uint32_t r = 0; r < rows; r++) {
+                const uint32_t slot = (r % K) * 32u + r / K;
+                for (uint32_t q = lane; q < kk; q += 32) out[(s0 + r) * n + j0 + q] = tile[slot * XS_ROW_WORDS + q];
+            }
+        }
+        __syncwarp();
+    }
+    if (live) store_words<K>(state + my0, w);
+    if (BULK && pending) bulk_wait_read_all(); // the tile must outlive the copies that read it
+}
+
+// In-register draw mode (row a6): {xor, sum} of n draws per stream.  The Weyl term is the
+// same for every word, so its sum is accumulated once per update and added at the end.
+template <int K, int THREADS>
+__global__ void __launch_bounds__(THREADS) xs1024_draw_kernel(Gen g, uint32_t *__restrict__ out, uint64_t n)
+{
+    constexpr int P = 32 / K;
+    constexpr int ROWS = 32 * K;
+    const int lane = threadIdx.x & 31;
+    const uint64_t wg = ((uint64_t)blockIdx.x * THREADS + threadIdx.x) >> 5;
+    const uint64_t s0 = wg * (uint64_t)ROWS;
+    if (s0 >= g.S) return; // warp-uniform
+    const int p = (P == 1) ? 0 : (lane & (P - 1));
+    const uint64_t my0 = s0 + (uint64_t)K * lane;
+    const bool live = my0 < g.S;
+    uint32_t *state = (uint32_t *)g.state;
+    uint32_t w[K], x[K], sm[K];
+#pragma unroll
+    for (int j = 0; j < K; j++) w[j] = 0u, x[j] = 0u, sm[j] = 0u;
+    if (live) load_words<K>(state + my0, w);
+    XsMasks<K> m;
+    m.init(p);
+    uint32_t nupd = (uint32_t)g.draws_done, wsum = 0u;
+#pragma unroll 1
+    for (uint64_t i = 0; i < n; i++) {
+        xs1024_update_k<K>(w, m);
+        nupd++;
+        const uint32_t wt = xs1024_weyl_term(nupd);
+        wsum += wt;
+#pragma unroll
+        for (int j = 0; j < K; j++) {
+            x[j] ^= wt + w[j];
+            sm[j] += w[j];
+        }
+    }
+    if (live) {
+        store_words<K>(state + my0, w);
+        uint32_t o[2 * K];
+#pragma unroll
+        for (int j = 0; j < K; j++) o[2 * j] = x[j], o[2 * j + 1] = sm[j] + wsum;
+        store_words<2 * K>(out + 2ull * my0, o);
+    }
+}
+
+template <int K, int WARPS, bool BULK>
+static cudaError_t launch_xs_fill(const Gen &g, uint32_t *o, uint64_t n, bool f32, cudaStream_t st)
+{
+    constexpr size_t smem = (size_t)WARPS * 32 * K * XS_ROW_WORDS * 4;
+    const uint64_t inst = g.S / 32, warps = (inst + K - 1) / K, grid = (warps + WARPS - 1) / WARPS;
+    if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+    static bool attr_set = false;
+    if (!attr_set && smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(xs1024_fill_kernel<K, true, WARPS, BULK>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(xs1024_fill_kernel<K, false, WARPS, BULK>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if (f32) xs1024_fill_kernel<K, true, WARPS, BULK><<<(unsigned)grid, WARPS * 32, smem, st>>>(g, o, n);
+    else xs1024_fill_kernel<K, false, WARPS, BULK><<<(unsigned)grid, WARPS * 32, smem, st>>>(g, o, n);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// variant "xs1024" = K (0: default); variant "store" = 1: LDS/STG write-out instead of TMA bulk stores
+cudaError_t launch_xs1024_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st)
+{
+    uint32_t *o = (uint32_t *)d_out;
+    const bool bulk = h.var_store != 1;
+#define XSF(K, WARPS) (bulk ? launch_xs_fill<K, WARPS, true>(h.g, o, n, f32, st) : launch_xs_fill<K, WARPS, false>(h.g, o, n, f32, st))
+    switch (h.var_xs1024) {
+    case 1: return XSF(1, 8);
+    case 2: return XSF(2, 4);
+    case 8: return XSF(8, 2);
+    case 16: return XSF(16, 1);
+    case 0:
+    case 4:
+    default: return XSF(4, 2);
+    }
+#undef XSF
+}
+
+template <int K, int THREADS>
+static cudaError_t launch_xs_draw(const Gen &g, uint32_t *o, uint64_t n, cudaStream_t st)
+{
+    const uint64_t inst = g.S / 32, warps = (inst + K - 1) / K, wpc = THREADS / 32, grid = (warps + wpc - 1) / wpc;
+    if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+    xs1024_draw_kernel<K, THREADS><<<(unsigned)grid, THREADS, 0, st>>>(g, o, n);
+    count_launch();
+    return cudaGetLastError();
+}
+
+cudaError_t launch_xs1024_draw(const rng_handle &h, uint32_t *d_out, uint64_t n, cudaStream_t st)
+{
+    // the API asks for 8-byte alignment only; K >= 2 stores 16-byte vectors
+    if (((uintptr_t)d_out & 15u) != 0u) return launch_xs_draw<1, 256>(h.g, d_out, n, st);
+    switch (h.var_xs1024) {
+    case 1: return launch_xs_draw<1, 256>(h.g, d_out, n, st);
+    case 2: return launch_xs_draw<2, 256>(h.g, d_out, n, st);
+    case 4: return launch_xs_draw<4, 256>(h.g, d_out, n, st);
+    case 8: return launch_xs_draw<8, 128>(h.g, d_out, n, st);
+    case 16: return launch_xs_draw<16, 128>(h.g, d_out, n, st);
+    case 0:
+    case 32:
+    default: return launch_xs_draw<32, 128>(h.g, d_out, n, st);
+    }
+}
+
+} // namespace rngb200

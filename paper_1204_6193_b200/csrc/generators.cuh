@@ -136,5 +136,10 @@ __host__ __device__ __forceinline__ uint32_t xs1024_weyl_term(uint64_t n_updates
 
 // fixed output map (BASELINE.json): (u >> 8) * 2^-24, exact (24-bit integer -> float)
 __device__ __forceinline__ float u32_to_f32(uint32_t u) { return __uint2float_rz(u >> 8) * 0x1p-24f; }
+// the 32-bit word a fill kernel stores: the draw itself, or the bits of its float image
+__device__ __forceinline__ uint32_t out_word(uint32_t u, bool f32)
+{
+    return f32 ? __float_as_uint(u32_to_f32(u)) : u;
+}
 
 } // namespace rngb200

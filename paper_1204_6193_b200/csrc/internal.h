@@ -56,6 +56,9 @@ void count_launch(uint64_t n = 1);
 cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st);
 // fill.cu  (f32 = apply the (u>>8)*2^-24 map; out is uint32_t* or float*)
 cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st);
+// fill_xs1024.cu (XORShift1024/Weyl, K words per lane; variant "xs1024" = K, 64 = the generic kernels)
+cudaError_t launch_xs1024_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st);
+cudaError_t launch_xs1024_draw(const rng_handle &h, uint32_t *d_out, uint64_t n, cudaStream_t st);
 // draw.cu
 cudaError_t launch_draw_reduce(const rng_handle &h, uint32_t *d_out, uint64_t n, cudaStream_t st);
 // ising.cu

@@ -116,6 +116,35 @@ def test_draw_reduce(kind, S, ns):
     g.close()
 
 
+@pytest.mark.parametrize("store", [0, 1], ids=["tma_bulk_store", "lds_stg"])
+@pytest.mark.parametrize("K", [1, 2, 4, 8, 16, 32, 64])
+def test_xs1024_lane_layouts_are_one_generator(K, store):
+    """the paper's generator with K words per lane (K = 1: Listing 1's one word per thread, shuffles;
+    K = 32: whole instance in one thread; 64: the generic row-tile / per-stream kernels): identical
+    fill (u32, f32, ragged n, unaligned rows), draw_reduce and final state"""
+    for S in (32, 32 * 37, 32 * 256 + 32 * 5):
+        g, o = pkg.Rng(pkg.RNG_XS1024W, S, 11), oracle.Rng(pkg.RNG_XS1024W, S, 11)
+        g.set_variant("xs1024", K)
+        g.set_variant("store", store)
+        for n in (64, 32, 5, 100, 1, 36, 128):
+            out = dev_u32(S * n)
+            g.fill_u32(out, n)
+            assert np.array_equal(host(out, S * n), o.fill_u32(n)), (K, S, n)
+        outf = torch.empty(S * 40, dtype=torch.float32, device="cuda")
+        g.fill_f32(outf, 40)
+        assert np.array_equal(outf.cpu().numpy().view(np.uint32), o.fill_f32(40).view(np.uint32))
+        for n in (257, 3, 0):
+            red = dev_u32(2 * S + 4)
+            g.draw_reduce(red, n)
+            assert np.array_equal(host(red, 2 * S), o.draw_reduce(n)), (K, S, n)
+        # 8-byte (not 16-byte) aligned checksum buffer is allowed by the API
+        pkg.rng_draw_reduce(g.handle, red.data_ptr() + 8, 9)
+        assert np.array_equal(host(red, 2 * S + 2)[2:], o.draw_reduce(9))
+        assert g.draws_done == o.draws_done
+        assert np.array_equal(g.get_state(), o.get_state())
+        g.close()
+
+
 # ---------------------------------------------------------------------------------
 # seeding / sharding: a shard [first, first+n_local) of n_total reproduces those rows
 # ---------------------------------------------------------------------------------
