@@ -13,41 +13,50 @@
 // memory and writes whole lines (a B200 microbenchmark of the alternative -- each thread
 // storing 32-byte row pieces directly -- reaches only 1.4 TB/s: partially written lines get
 // evicted from L2).  See xs1024_fill_kernel for the tile layout and the TMA bulk-store write-out.
+#include <cstring>
+
+#include <cuda.h>
+
 #include "internal.h"
 #include "xs1024.cuh"
 
 namespace rngb200 {
 
-// ---- TMA bulk store of one staged row (shared -> global), issued by the lane that wrote it ----
-__device__ __forceinline__ void bulk_store_row(uint32_t *gdst, const uint32_t *ssrc, uint32_t bytes)
+// ---- TMA tensor store of a staged tile (shared -> global) ----
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap *tm, const uint32_t *ssrc, int c0, int c1, int c2)
 {
     const uint32_t saddr = (uint32_t)__cvta_generic_to_shared(ssrc);
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(saddr), "r"(bytes)
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(tm), "r"(saddr),
+                 "r"(c0), "r"(c1), "r"(c2)
                  : "memory");
 }
-__device__ __forceinline__ void bulk_fence_generic_to_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_generic_to_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
-constexpr int XS_ROW_WORDS = 36; // staged row: 32 draws + 4 words of padding (16-byte aligned, conflict-free)
-
-// Tile layout: row r = K*lane + j of the warp sits in slot j*32 + lane, slots are XS_ROW_WORDS
-// apart: the 128-bit stores of the eight lanes of a quarter-warp hit eight different bank
-// groups, and a staged row is contiguous, as a bulk copy needs.
-// BULK: every lane hands its own K rows to the TMA unit (cp.async.bulk shared -> global, one
-// 128-byte line per copy) and goes on generating; it waits for the copies to have READ the
-// tile only just before it overwrites it.  No warp synchronisation, no LDS/STG write-out.
-// !BULK (and every ragged or unaligned tile): write-out with LDS.128 + streaming STG.128.
-template <int K, bool F32, int WARPS, bool BULK>
-__global__ void __launch_bounds__(WARPS * 32) xs1024_fill_kernel(Gen g, uint32_t *__restrict__ out, uint64_t n)
+// Tile layout (per warp, 1 KiB aligned): row r = K*lane + j of the warp's 32K rows sits in
+// slot j*32 + lane; a slot is 128 dense bytes = the row's 32 draws; its eight 16-byte chunks
+// are XOR-swizzled with slot & 7 = lane & 7.  The generating 128-bit stores of a quarter-warp
+// then hit eight different bank groups, the write-out loads (eight lanes -> the eight chunks
+// of one row) are conflict-free, and the layout is exactly TMA's SWIZZLE_128B box of a
+// rank-3 tensor map over the output with dimensions (draw, row / K, row % K).
+// TMA: lane 0 hands the whole tile to the TMA unit with ONE cp.async.bulk.tensor (shared ->
+// global; columns past n and rows past S are clipped by the unit, so ragged tiles need no
+// special case) and the warp goes on generating; it waits for the copy to have READ the tile
+// only just before overwriting it.  No LDS/STG write-out at all.
+// !TMA (and rows that are not 16-byte aligned, n % 4 != 0): LDS.128 + streaming STG.128.
+template <int K, bool F32, int WARPS, bool TMA>
+__global__ void __launch_bounds__(WARPS * 32)
+    xs1024_fill_kernel(Gen g, uint32_t *__restrict__ out, uint64_t n, const __grid_constant__ CUtensorMap tmap)
 {
-    extern __shared__ __align__(16) uint32_t xs_tiles[];
+    extern __shared__ __align__(1024) uint32_t xs_tiles[];
     constexpr int P = 32 / K;
     constexpr int ROWS = 32 * K;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t *tile = xs_tiles + warp * (ROWS * XS_ROW_WORDS);
-    const uint64_t s0 = ((uint64_t)blockIdx.x * WARPS + warp) * (uint64_t)ROWS; // first row of this warp
-    if (s0 >= g.S) return;                                                      // warp-uniform
+    uint32_t *tile = xs_tiles + warp * (ROWS * 32);
+    const uint64_t wg = (uint64_t)blockIdx.x * WARPS + warp;
+    const uint64_t s0 = wg * (uint64_t)ROWS; // first row of this warp
+    if (s0 >= g.S) return;                   // warp-uniform
     const int p = (P == 1) ? 0 : (lane & (P - 1));
     const uint64_t my0 = s0 + (uint64_t)K * lane; // S % 32 == 0 and K | 32: my K rows are all live or all dead
     const bool live = my0 < g.S;
@@ -62,9 +71,9 @@ __global__ void __launch_bounds__(WARPS * 32) xs1024_fill_kernel(Gen g, uint32_t
     XsMasks<K> m;
     m.init(p);
     uint32_t nupd = (uint32_t)g.draws_done; // the Weyl term only needs the update count mod 2^32
-    uint32_t *myrows = tile + lane * XS_ROW_WORDS; // + j * 32 * XS_ROW_WORDS
-    uint32_t *grow = out + my0 * n;                // my first row in the output
-    bool pending = false;                          // bulk copies of mine may still be reading the tile
+    const uint32_t swz = (uint32_t)lane & 7u;
+    uint32_t *myrows = tile + lane * 32; // + j * 32 * 32
+    bool pending = false;               // a tensor store may still be reading the tile
 
     for (uint64_t j0 = 0; j0 < n; j0 += 32) {
         const uint32_t kk = (uint32_t)((n - j0 < 32ull) ? (n - j0) : 32ull);
@@ -80,18 +89,20 @@ __global__ void __launch_bounds__(WARPS * 32) xs1024_fill_kernel(Gen g, uint32_t
 #pragma unroll
                 for (int j = 0; j < K; j++) o[j][u] = out_word(wt + w[j], F32);
             }
-            if (BULK && pending) {
-                bulk_wait_read_all();
+            if (TMA && pending) { // warp-uniform
+                if (lane == 0) bulk_wait_read_all();
+                __syncwarp();
                 pending = false;
             }
+            const uint32_t phys = (c ^ swz) * 4u;
 #pragma unroll
             for (int j = 0; j < K; j++)
-                *reinterpret_cast<uint4 *>(myrows + j * (32 * XS_ROW_WORDS) + 4u * c) =
-                    make_uint4(o[j][0], o[j][1], o[j][2], o[j][3]);
+                *reinterpret_cast<uint4 *>(myrows + j * 1024 + phys) = make_uint4(o[j][0], o[j][1], o[j][2], o[j][3]);
         }
         if (4u * c < kk) { // ragged tail of the call
-            if (BULK && pending) {
-                bulk_wait_read_all();
+            if (TMA && pending) {
+                if (lane == 0) bulk_wait_read_all();
+                __syncwarp();
                 pending = false;
             }
             for (uint32_t u = 4u * c; u < kk; u++) {
@@ -99,18 +110,18 @@ __global__ void __launch_bounds__(WARPS * 32) xs1024_fill_kernel(Gen g, uint32_t
                 nupd++;
                 const uint32_t wt = xs1024_weyl_term(nupd);
 #pragma unroll
-                for (int j = 0; j < K; j++) myrows[j * (32 * XS_ROW_WORDS) + u] = out_word(wt + w[j], F32);
+                for (int j = 0; j < K; j++) myrows[j * 1024 + ((u >> 2) ^ swz) * 4u + (u & 3u)] = out_word(wt + w[j], F32);
             }
         }
-        if (BULK && kk == 32u && vec_ok) {
-            // ---- hand my K rows to the TMA unit: 128 contiguous bytes each ----
-            if (live) {
-                bulk_fence_generic_to_async();
-#pragma unroll
-                for (int j = 0; j < K; j++) bulk_store_row(grow + (uint64_t)j * n + j0, myrows + j * (32 * XS_ROW_WORDS), 128u);
+        if (TMA && vec_ok) {
+            // ---- one tensor store for the whole tile: box (32 draws, 32 lanes, K words) ----
+            fence_generic_to_async(); // my generic-proxy writes -> visible to the async proxy
+            __syncwarp();
+            if (lane == 0) {
+                tma_store_3d(&tmap, tile, (int)j0, (int)(wg * 32ull), 0);
                 bulk_commit();
-                pending = true;
             }
+            pending = true;
             continue;
         }
         __syncwarp();
@@ -125,27 +136,28 @@ __global__ void __launch_bounds__(WARPS * 32) xs1024_fill_kernel(Gen g, uint32_t
                 for (int it = 0; it < 8 * K; it++) {
                     const uint32_t r = 4u * (uint32_t)it + r0;
                     const uint32_t slot = (r % K) * 32u + r / K;
-                    const uint4 v = *reinterpret_cast<const uint4 *>(tile + slot * XS_ROW_WORDS + 4u * ch);
+                    const uint4 v = *reinterpret_cast<const uint4 *>(tile + slot * 32u + ((ch ^ (slot & 7u)) * 4u));
                     __stcs(reinterpret_cast<uint4 *>(gp), v);
                     gp += gstep;
                 }
             } else {
                 for (uint32_t r = r0; r < rows; r += 4u, gp += gstep) {
                     const uint32_t slot = (r % K) * 32u + r / K;
-                    const uint4 v = *reinterpret_cast<const uint4 *>(tile + slot * XS_ROW_WORDS + 4u * ch);
+                    const uint4 v = *reinterpret_cast<const uint4 *>(tile + slot * 32u + ((ch ^ (slot & 7u)) * 4u));
                     __stcs(reinterpret_cast<uint4 *>(gp), v);
                 }
             }
         } else {
             for (uint32_t r = 0; r < rows; r++) {
                 const uint32_t slot = (r % K) * 32u + r / K;
-                for (uint32_t q = lane; q < kk; q += 32) out[(s0 + r) * n + j0 + q] = tile[slot * XS_ROW_WORDS + q];
+                for (uint32_t q = lane; q < kk; q += 32)
+                    out[(s0 + r) * n + j0 + q] = tile[slot * 32u + (((q >> 2) ^ (slot & 7u)) * 4u) + (q & 3u)];
             }
         }
         __syncwarp();
     }
     if (live) store_words<K>(state + my0, w);
-    if (BULK && pending) bulk_wait_read_all(); // the tile must outlive the copies that read it
+    if (TMA && pending && lane == 0) bulk_wait_read_all(); // the tile must outlive the copy that reads it
 }
 
 // In-register draw mode (row a6): {xor, sum} of n draws per stream.  The Weyl term is the
@@ -191,41 +203,80 @@ __global__ void __launch_bounds__(THREADS) xs1024_draw_kernel(Gen g, uint32_t *_
     }
 }
 
-template <int K, int WARPS, bool BULK>
-static cudaError_t launch_xs_fill(const Gen &g, uint32_t *o, uint64_t n, bool f32, cudaStream_t st)
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn()
 {
-    constexpr size_t smem = (size_t)WARPS * 32 * K * XS_ROW_WORDS * 4;
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// rank-3 view of the stream-major output out[row*n + draw], row = K*l + j:
+// dimensions (draw: n, l: S/K, j: K), box (32, 32, K), SWIZZLE_128B
+static bool make_out_tensor_map(CUtensorMap *tm, uint32_t *out, uint64_t S, uint64_t n, int K)
+{
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc || (n & 3ull) || n > 0xffffffffull || ((uintptr_t)out & 15u)) return false;
+    const cuuint64_t dims[3] = {n, S / (uint64_t)K, (cuuint64_t)K};
+    const cuuint64_t strides[2] = {(cuuint64_t)K * n * 4ull, n * 4ull};
+    if (strides[0] >= (1ull << 40)) return false;
+    const cuuint32_t box[3] = {32u, 32u, (cuuint32_t)K};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, out, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) ==
+           CUDA_SUCCESS;
+}
+
+template <int K, int WARPS, bool TMA>
+static cudaError_t launch_xs_fill(const Gen &g, uint32_t *o, uint64_t n, bool f32, const CUtensorMap &tm, cudaStream_t st)
+{
+    constexpr size_t smem = (size_t)WARPS * 32 * K * 32 * 4;
     const uint64_t inst = g.S / 32, warps = (inst + K - 1) / K, grid = (warps + WARPS - 1) / WARPS;
     if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
     static bool attr_set = false;
     if (!attr_set && smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(xs1024_fill_kernel<K, true, WARPS, BULK>,
+        cudaError_t e = cudaFuncSetAttribute(xs1024_fill_kernel<K, true, WARPS, TMA>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(xs1024_fill_kernel<K, false, WARPS, BULK>,
+            e = cudaFuncSetAttribute(xs1024_fill_kernel<K, false, WARPS, TMA>,
                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    if (f32) xs1024_fill_kernel<K, true, WARPS, BULK><<<(unsigned)grid, WARPS * 32, smem, st>>>(g, o, n);
-    else xs1024_fill_kernel<K, false, WARPS, BULK><<<(unsigned)grid, WARPS * 32, smem, st>>>(g, o, n);
+    if (f32) xs1024_fill_kernel<K, true, WARPS, TMA><<<(unsigned)grid, WARPS * 32, smem, st>>>(g, o, n, tm);
+    else xs1024_fill_kernel<K, false, WARPS, TMA><<<(unsigned)grid, WARPS * 32, smem, st>>>(g, o, n, tm);
     count_launch();
     return cudaGetLastError();
 }
 
-// variant "xs1024" = K (0: default); variant "store" = 1: LDS/STG write-out instead of TMA bulk stores
+// variant "xs1024" = K (0: default); variant "store": 0 = default, 1 = LDS/STG write-out, 2 = TMA tensor store
 cudaError_t launch_xs1024_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st)
 {
     uint32_t *o = (uint32_t *)d_out;
-    const bool bulk = h.var_store != 1;
-#define XSF(K, WARPS) (bulk ? launch_xs_fill<K, WARPS, true>(h.g, o, n, f32, st) : launch_xs_fill<K, WARPS, false>(h.g, o, n, f32, st))
-    switch (h.var_xs1024) {
+    const int K = (h.var_xs1024 == 1 || h.var_xs1024 == 2 || h.var_xs1024 == 8 || h.var_xs1024 == 16) ? h.var_xs1024 : 4;
+    alignas(64) CUtensorMap tm;
+    memset(&tm, 0, sizeof tm);
+    const bool tma = h.var_store != 1 && make_out_tensor_map(&tm, o, h.g.S, n, K);
+#define XSF(KK, WARPS) \
+    (tma ? launch_xs_fill<KK, WARPS, true>(h.g, o, n, f32, tm, st) : launch_xs_fill<KK, WARPS, false>(h.g, o, n, f32, tm, st))
+    switch (K) {
     case 1: return XSF(1, 8);
     case 2: return XSF(2, 4);
     case 8: return XSF(8, 2);
     case 16: return XSF(16, 1);
-    case 0:
-    case 4:
     default: return XSF(4, 2);
     }
 #undef XSF
