@@ -361,6 +361,7 @@ int rng_set_variant(rng_handle *h, const char *name, int value)
     if (!strcmp(name, "xs1024")) h->var_xs1024 = value;
     else if (!strcmp(name, "ising")) h->var_ising = value;
     else if (!strcmp(name, "store")) h->var_store = value;
+    else if (!strcmp(name, "lcg")) h->var_lcg = value;
     else return fail(RNG_E_INVAL, "rng_set_variant: unknown name '%s'", name);
     return RNG_OK;
 }

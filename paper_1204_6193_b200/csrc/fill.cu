@@ -102,13 +102,13 @@ __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_
             c2[u] = n2;
         }
     }
+    uint4 *dst = reinterpret_cast<uint4 *>(row) + rb0; // one address per lane; the U stores use immediate offsets
 #pragma unroll
     for (int u = 0; u < U; u++) {
-        const uint32_t rb = rb0 + 32u * u;
-        if (!CHECK || rb < blocks_per_row) {
+        if (!CHECK || rb0 + 32u * u < blocks_per_row) {
             const uint4 v = make_uint4(out_word(c0[u], F32), out_word(c1[u], F32), out_word(c2[u], F32),
                                        out_word(c3[u], F32));
-            __stcs(reinterpret_cast<uint4 *>(row + 4ull * rb), v); // streaming 128-bit store
+            __stcs(dst + 32 * u, v); // streaming 128-bit store
         }
     }
 }
@@ -233,6 +233,66 @@ __global__ void __launch_bounds__(FILL_WARPS * 32) rowtile_fill_kernel(Gen g, ui
     if (live) gen.store(g, s);
 }
 
+// ------------------------------------------------------------------------------------
+// LCG64 with FEW streams (BASELINE config 1: 1024 streams x 4096 draws): one thread per
+// stream would leave the chip empty and serialise 4096 dependent multiplies per thread.
+// The paper's skip-ahead (eq.(2)) is applied INSIDE each stream instead:
+// one CTA per stream, lane t starts at x_{4t} = step^(4t)(x_0) (table mult4, built by the
+// seeding kernel), writes draws 4t..4t+3 with one 128-bit store and leaps by
+// step^1024 = pow2[10] to its next chunk.  Same bits as the sequential walk, coalesced for
+// free (a warp instruction stores 512 contiguous bytes).  Thread 0 writes the stream's final
+// state x_n = step^n(x_0), composed from the pow2 table over the bits of n.
+// ------------------------------------------------------------------------------------
+template <bool F32>
+__global__ void __launch_bounds__(256) lcg_intra_fill_kernel(Gen g, uint32_t *__restrict__ out, uint64_t n)
+{
+    const uint64_t s = blockIdx.x;
+    const uint32_t t = threadIdx.x;
+    const LcgTable *__restrict__ tab = g.lcg;
+    uint64_t *xs = (uint64_t *)g.state;
+    const uint64_t x0 = xs[s];
+    const Affine step = tab->pow2[0], leap = tab->pow2[10];
+    uint64_t x = affine_apply(tab->mult4[t], x0); // x_{4t}
+    uint32_t *row = out + s * n;
+    const bool vec_ok = (n & 3ull) == 0ull;
+    for (uint64_t j = 4ull * t; j < n; j += 1024ull) {
+        uint64_t y = x;
+        uint4 v;
+        v.x = out_word((uint32_t)(y >> 32), F32); // 32 most significant bits
+        y = affine_apply(step, y);
+        v.y = out_word((uint32_t)(y >> 32), F32);
+        y = affine_apply(step, y);
+        v.z = out_word((uint32_t)(y >> 32), F32);
+        y = affine_apply(step, y);
+        v.w = out_word((uint32_t)(y >> 32), F32);
+        if (vec_ok) {
+            __stcs(reinterpret_cast<uint4 *>(row + j), v);
+        } else {
+            row[j] = v.x;
+            if (j + 1 < n) row[j + 1] = v.y;
+            if (j + 2 < n) row[j + 2] = v.z;
+            if (j + 3 < n) row[j + 3] = v.w;
+        }
+        x = affine_apply(leap, x);
+    }
+    __syncthreads(); // every lane has read xs[s]
+    if (t == 0) {
+        uint64_t y = x0;
+        for (int m = 0; m < 64 && (n >> m) != 0ull; m++)
+            if ((n >> m) & 1ull) y = affine_apply(tab->pow2[m], y);
+        xs[s] = y;
+    }
+}
+
+static cudaError_t launch_lcg_intra(const Gen &g, void *d_out, uint64_t n, bool f32, cudaStream_t st)
+{
+    if (g.S > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+    if (f32) lcg_intra_fill_kernel<true><<<(unsigned)g.S, 256, 0, st>>>(g, (uint32_t *)d_out, n);
+    else lcg_intra_fill_kernel<false><<<(unsigned)g.S, 256, 0, st>>>(g, (uint32_t *)d_out, n);
+    count_launch();
+    return cudaGetLastError();
+}
+
 static int g_sm_count = 0;
 static int sm_count()
 {
@@ -324,6 +384,11 @@ static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, boo
 cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st)
 {
     const Gen &g = h.g;
+    if (g.kind == RNG_LCG64 || g.kind == RNG_LCG64_LEAPFROG) {
+        // variant "lcg": 0 = automatic, 1 = one thread per stream (row tiles), 2 = one CTA per stream
+        const bool few = g.S < 65536ull && n >= 512ull;
+        if (h.var_lcg == 2 || (h.var_lcg == 0 && few)) return launch_lcg_intra(g, d_out, n, f32, st);
+    }
     switch (g.kind) {
     case RNG_LCG64: return launch_rowtile<RNG_LCG64>(g, d_out, n, f32, h.var_store, st);
     case RNG_LCG64_LEAPFROG: return launch_rowtile<RNG_LCG64_LEAPFROG>(g, d_out, n, f32, h.var_store, st);

@@ -135,7 +135,18 @@ __host__ __device__ __forceinline__ uint32_t xs1024_weyl_term(uint64_t n_updates
 }
 
 // fixed output map (BASELINE.json): (u >> 8) * 2^-24, exact (24-bit integer -> float)
-__device__ __forceinline__ float u32_to_f32(uint32_t u) { return __uint2float_rz(u >> 8) * 0x1p-24f; }
+// Evaluated without the integer->float conversion unit (I2FP issues at a quarter of the FFMA
+// rate on sm_100a and shares a pipe with Philox's IMAD.WIDE): with u = b3 b2 b1 b0 (bytes),
+//   A = 0x4B00'b3b2 = 2^23 + (u >> 16),   B = 0x4B00'00b1 = 2^23 + ((u >> 8) & 255)   (one PRMT each)
+//   f = fma(B, 2^-24, fma(A, 2^-16, -128.5))
+// The inner fma is (u>>16) 2^-16 - 1/2 and the outer one adds 1/2 + b1 2^-24; both results
+// are representable, so no rounding occurs anywhere and f == (float)(u >> 8) * 2^-24 bit for bit.
+__device__ __forceinline__ float u32_to_f32(uint32_t u)
+{
+    const float A = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7432));
+    const float B = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7441));
+    return __fmaf_rn(B, 0x1p-24f, __fmaf_rn(A, 0x1p-16f, -128.5f));
+}
 // the 32-bit word a fill kernel stores: the draw itself, or the bits of its float image
 __device__ __forceinline__ uint32_t out_word(uint32_t u, bool f32)
 {

@@ -45,7 +45,7 @@ struct rng_handle {
     int64_t *energy_scratch; // device, 1 x int64
     uint32_t *ms_planes;     // device scratch of the multi-spin Ising path: two bit planes of L*L/64 words
     uint64_t ms_planes_bytes;
-    int var_xs1024, var_ising, var_store;
+    int var_xs1024, var_ising, var_store, var_lcg;
 };
 
 namespace rngb200 {

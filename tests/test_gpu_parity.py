@@ -116,7 +116,27 @@ def test_draw_reduce(kind, S, ns):
     g.close()
 
 
-@pytest.mark.parametrize("store", [0, 1], ids=["tma_bulk_store", "lds_stg"])
+@pytest.mark.parametrize("kind", [pkg.RNG_LCG64, pkg.RNG_LCG64_LEAPFROG], ids=["lcg64", "lcg64_leapfrog"])
+@pytest.mark.parametrize("variant", [1, 2], ids=["thread_per_stream", "cta_per_stream"])
+def test_lcg_intra_stream_skip_ahead_is_the_same_stream(kind, variant):
+    """eq.(2) applied inside a stream (one CTA per stream, lanes leap by step^1024) gives the bits of
+    the sequential walk: u32, f32, ragged and unaligned n, continuation, final state"""
+    S = 37
+    g, o = pkg.Rng(kind, S, 5), oracle.Rng(kind, S, 5)
+    g.set_variant("lcg", variant)
+    for n in (4096, 1024, 1, 3, 1030, 2047, 0, 512):
+        out = dev_u32(S * n)
+        g.fill_u32(out, n)
+        assert np.array_equal(host(out, S * n), o.fill_u32(n)), (variant, n)
+        assert np.array_equal(g.get_state(), o.get_state()), (variant, n)
+    outf = torch.empty(S * 1500, dtype=torch.float32, device="cuda")
+    g.fill_f32(outf, 1500)
+    assert np.array_equal(outf.cpu().numpy().view(np.uint32), o.fill_f32(1500).view(np.uint32))
+    assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
+
+
+@pytest.mark.parametrize("store", [0, 1], ids=["tma_tensor_store", "lds_stg"])
 @pytest.mark.parametrize("K", [1, 2, 4, 8, 16, 32, 64])
 def test_xs1024_lane_layouts_are_one_generator(K, store):
     """the paper's generator with K words per lane (K = 1: Listing 1's one word per thread, shuffles;
