@@ -102,6 +102,8 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
     h->g.n_total = n_total;
     h->g.seed = seed;
     h->g.draws_done = 0;
+    h->g.k_one = 1u;
+    h->g.k_zero = 0u;
     h->state_bytes = rng_state_bytes(kind, n_local);
     cudaError_t e = cudaSuccess;
     LcgTable *tab = nullptr;

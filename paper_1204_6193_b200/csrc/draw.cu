@@ -7,28 +7,41 @@
 
 namespace rngb200 {
 
+// UNROLL draws per trip of the main loop.  XORWOW rotates its five words every draw, so a
+// multiple of 5 lets the compiler rename registers instead of moving them.
 template <int KIND>
 __global__ void __launch_bounds__(256) draw_reduce_kernel(Gen g, uint2 *__restrict__ out, uint64_t n)
 {
+    constexpr int UNROLL = (KIND == RNG_XORWOW) ? 20 : 8;
     const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= g.S) return; // xs1024: S % 32 == 0, whole warps leave together
     Stream<KIND> gen;
     gen.load(g, s);
     uint32_t x = 0u, sum = 0u;
-    uint64_t j = 0;
-    for (; j + 4 <= n; j += 4) {
+    // XORWOW's draw is 4-5 alu-pipe operations (xors, the right shift) and as many additions /
+    // left shifts; with the additions pinned to the fma pipe the two pipes carry equal loads.
+    const uint32_t one = g.k_one;
+    auto draw = [&]() -> uint32_t {
+        if constexpr (KIND == RNG_XORWOW) return gen.st.next_fma_adds(one);
+        else return gen.next();
+    };
+    auto accumulate = [&](uint32_t u) {
+        x ^= u;
+        if constexpr (KIND == RNG_XORWOW) sum = add_on_fma_pipe(sum, u, one);
+        else sum += u;
+    };
+    uint64_t trips = n / UNROLL;
+    const uint32_t rest = (uint32_t)(n - trips * UNROLL);
+    while (trips) { // 32-bit inner counter: the 64-bit one costs three uniform instructions per trip
+        const uint32_t t32 = trips > 0x40000000ull ? 0x40000000u : (uint32_t)trips;
+        trips -= t32;
+#pragma unroll 1
+        for (uint32_t t = 0; t < t32; t++) {
 #pragma unroll
-        for (int q = 0; q < 4; q++) {
-            const uint32_t u = gen.next();
-            x ^= u;
-            sum += u;
+            for (int q = 0; q < UNROLL; q++) accumulate(draw());
         }
     }
-    for (; j < n; j++) {
-        const uint32_t u = gen.next();
-        x ^= u;
-        sum += u;
-    }
+    for (uint32_t j = 0; j < rest; j++) accumulate(draw());
     gen.store(g, s);
     out[s] = make_uint2(x, sum);
 }

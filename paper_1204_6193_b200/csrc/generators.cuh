@@ -51,6 +51,15 @@ __host__ __device__ inline Affine affine_pow(Affine base, uint64_t n)
 // ---------------------------------------------------------------------------------
 // XORWOW (R-B1).  State words x,y,z,w,v and Weyl counter d; advance, then output.
 // ---------------------------------------------------------------------------------
+// Pipe steering (sm_100a): LOP3, SHF and IADD3 issue on the alu pipe, IMAD (non-wide) on the
+// fma pipe, 64 lanes/clk/SM each.  ptxas decides between IADD3 and IMAD.IADD by its own
+// heuristics; where a kernel is bound by one of the two pipes these helpers pin an addition
+// to the other one.  `one` / `zero` are the kernel parameters Gen::k_one / Gen::k_zero (1 and 0,
+// which neither nvvm nor ptxas can fold), so  a*one + b  must stay an IMAD and the
+// three-input  a + b + zero  an IADD3.
+__device__ __forceinline__ uint32_t add_on_fma_pipe(uint32_t a, uint32_t b, uint32_t one) { return a * one + b; }
+__device__ __forceinline__ uint32_t add_on_alu_pipe(uint32_t a, uint32_t b, uint32_t zero) { return a + b + zero; }
+
 struct Xorwow {
     uint32_t x, y, z, w, v, d;
     __device__ __forceinline__ uint32_t next()
@@ -60,6 +69,15 @@ struct Xorwow {
         v = (v ^ (v << 4)) ^ (t ^ (t << 1));
         d += 362437u;
         return d + v;
+    }
+    // same draw with the two additions pinned to the fma pipe (for alu-pipe-bound consumers)
+    __device__ __forceinline__ uint32_t next_fma_adds(uint32_t one)
+    {
+        uint32_t t = x ^ (x >> 2);
+        x = y; y = z; z = w; w = v;
+        v = (v ^ (v << 4)) ^ (t ^ (t << 1));
+        d = add_on_fma_pipe(d, 362437u, one);
+        return add_on_fma_pipe(d, v, one);
     }
 };
 

@@ -32,6 +32,9 @@ struct Gen {
     uint64_t draws_done; // per stream, all streams in lockstep
     void *state;         // device
     const LcgTable *lcg; // device (LCG kinds only)
+    // the constants 1 and 0 as kernel parameters: values ptxas cannot fold, used to pin an
+    // addition to the fma pipe (a*one + b) or the alu pipe (a + b + zero); see generators.cuh
+    uint32_t k_one, k_zero;
 };
 
 } // namespace rngb200

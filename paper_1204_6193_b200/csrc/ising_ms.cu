@@ -125,12 +125,18 @@ __global__ void __launch_bounds__(64) ising_ms_stream_kernel(Gen g, uint32_t *__
     } else {
         Stream<KIND> gen;
         gen.load(g, s);
+        const uint32_t one = g.k_one; // the compares fill the alu pipe: XORWOW's additions go to the fma pipe
         for (uint32_t i = 0; i < W; i++) {
             MsWord mw;
             mw.load(Cp, Np, L, wpr, y, j, colour);
             uint32_t n0 = 0u, n1 = 0u;
 #pragma unroll
-            for (int k = 0; k < 32; k++) ms_cmp_insert(gen.next(), thr, n0, n1);
+            for (int k = 0; k < 32; k++) {
+                uint32_t r;
+                if constexpr (KIND == RNG_XORWOW) r = gen.st.next_fma_adds(one);
+                else r = gen.next();
+                ms_cmp_insert(r, thr, n0, n1);
+            }
             mw.update_store(n0, n1);
             if (++j == wpr) {
                 j = 0;
@@ -169,12 +175,18 @@ __global__ void __launch_bounds__(128) ising_ms_word_kernel(Gen g, uint32_t *__r
             ms_cmp_insert(o.w, thr, n0, n1);
         }
     } else {
+        const uint32_t one = g.k_one;
 #pragma unroll
         for (int a = 0; a < 32 / K; a++) {
             Stream<KIND> gen;
             gen.load(g, s0 + a);
 #pragma unroll
-            for (int k = 0; k < K; k++) ms_cmp_insert(gen.next(), thr, n0, n1);
+            for (int k = 0; k < K; k++) {
+                uint32_t r;
+                if constexpr (KIND == RNG_XORWOW) r = gen.st.next_fma_adds(one);
+                else r = gen.next();
+                ms_cmp_insert(r, thr, n0, n1);
+            }
             gen.store(g, s0 + a);
         }
     }
