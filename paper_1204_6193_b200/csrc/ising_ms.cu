@@ -147,6 +147,33 @@ __global__ void __launch_bounds__(64) ising_ms_stream_kernel(Gen g, uint32_t *__
     }
 }
 
+// N consecutive 32-bit words, 4N-byte aligned (N = 2, 4, 8)
+template <int N>
+__device__ __forceinline__ void load_vec(const uint32_t *__restrict__ p, uint32_t (&v)[N])
+{
+    if constexpr (N == 2) {
+        const uint2 t = *reinterpret_cast<const uint2 *>(p);
+        v[0] = t.x, v[1] = t.y;
+    } else {
+#pragma unroll
+        for (int q = 0; q < N / 4; q++) {
+            const uint4 t = reinterpret_cast<const uint4 *>(p)[q];
+            v[4 * q] = t.x, v[4 * q + 1] = t.y, v[4 * q + 2] = t.z, v[4 * q + 3] = t.w;
+        }
+    }
+}
+template <int N>
+__device__ __forceinline__ void store_vec(uint32_t *__restrict__ p, const uint32_t (&v)[N])
+{
+    if constexpr (N == 2) {
+        *reinterpret_cast<uint2 *>(p) = make_uint2(v[0], v[1]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < N / 4; q++)
+            reinterpret_cast<uint4 *>(p)[q] = make_uint4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+    }
+}
+
 // ---- WORD mode: K in {4, 8, 16}, 32/K streams per word -------------------------------
 template <int KIND, int K>
 __global__ void __launch_bounds__(128) ising_ms_word_kernel(Gen g, uint32_t *__restrict__ Cp,
@@ -174,19 +201,31 @@ __global__ void __launch_bounds__(128) ising_ms_word_kernel(Gen g, uint32_t *__r
             ms_cmp_insert(o.z, thr, n0, n1);
             ms_cmp_insert(o.w, thr, n0, n1);
         }
-    } else {
+    } else if constexpr (KIND == RNG_XORWOW) {
+        // the 32/K streams of this word are consecutive in the interleaved state w[k*S + s]:
+        // one vector load / store per state word instead of one access per stream and word
+        constexpr int NS = 32 / K;
         const uint32_t one = g.k_one;
+        uint32_t *w = (uint32_t *)g.state;
+        uint32_t st[6][NS];
+#pragma unroll
+        for (int k = 0; k < 6; k++) load_vec<NS>(w + (uint64_t)k * g.S + s0, st[k]);
+#pragma unroll
+        for (int a = 0; a < NS; a++) {
+            Xorwow x{st[0][a], st[1][a], st[2][a], st[3][a], st[4][a], st[5][a]};
+#pragma unroll
+            for (int k = 0; k < K; k++) ms_cmp_insert(x.next_fma_adds(one), thr, n0, n1);
+            st[0][a] = x.x, st[1][a] = x.y, st[2][a] = x.z, st[3][a] = x.w, st[4][a] = x.v, st[5][a] = x.d;
+        }
+#pragma unroll
+        for (int k = 0; k < 6; k++) store_vec<NS>(w + (uint64_t)k * g.S + s0, st[k]);
+    } else {
 #pragma unroll
         for (int a = 0; a < 32 / K; a++) {
             Stream<KIND> gen;
             gen.load(g, s0 + a);
 #pragma unroll
-            for (int k = 0; k < K; k++) {
-                uint32_t r;
-                if constexpr (KIND == RNG_XORWOW) r = gen.st.next_fma_adds(one);
-                else r = gen.next();
-                ms_cmp_insert(r, thr, n0, n1);
-            }
+            for (int k = 0; k < K; k++) ms_cmp_insert(gen.next(), thr, n0, n1);
             gen.store(g, s0 + a);
         }
     }
