@@ -47,15 +47,31 @@ def measured_peaks() -> dict:
 N_SM, SMSP_PER_SM, LANES = 148, 4, 32  # B200: 148 SMs x 4 schedulers x 1 warp-instruction/clk
 
 
+def measured_traffic(name: str):
+    """DRAM bytes per launch of the workload's dominant kernel from the committed `ncu --set full`
+    capture (profiles/traffic.json, written from the raw page; never measured under this run)"""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p)).get(name, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
 def issue_peak_tinst(sm_mhz: float) -> float:
     """thread-instruction issue peak in Tinst/s ('alu' roofline)"""
     return N_SM * SMSP_PER_SM * LANES * sm_mhz * 1e6 / 1e12
 
 
-# algorithmic thread-instructions per draw (DESIGN.md section 7 derives each count
-# from the recurrences as written in the paper, not from the compiled SASS)
-ALG_INST_PER_DRAW = {W.LCG64: 5.0, W.LCG64_LEAPFROG: 5.0, W.XORWOW: 10.0, W.PHILOX4X32_10: 12.0, W.XS1024W: 17.0}
-ALG_INST_PER_ISING_UPDATE = 12.0   # neighbour loads+sum, h, table select, compare, flip, store (excl. the draw)
+# algorithmic thread-instructions per draw (DESIGN.md section 7 derives each count from the
+# recurrences as written in the paper, not from the compiled SASS): LCG64 = 64-bit multiply-add
+# in 32-bit pieces (3) + checksum (2); XORWOW = 3 shifts + 3 xors + 2 adds + checksum (2);
+# Philox = per word 5 mulhi/lo + 5 xors + key/counter (2); xs1024 register-resident = 66 funnel
+# shifts + 66 xors per 32 words (the zero padding drops 10 of 32 words per phase) + Weyl add (1)
+# + checksum (2)
+ALG_INST_PER_DRAW = {W.LCG64: 5.0, W.LCG64_LEAPFROG: 5.0, W.XORWOW: 10.0, W.PHILOX4X32_10: 12.0, W.XS1024W: 7.0}
+# multi-spin-coded update: two threshold compares of two instructions each + the bit-sliced
+# neighbour count / flip logic amortised over the 32 sites of a word (about 1), excl. the draw
+ALG_INST_PER_ISING_UPDATE = 5.0
 STATE_BYTES = {W.LCG64: 8, W.LCG64_LEAPFROG: 8, W.XORWOW: 24, W.PHILOX4X32_10: 0, W.XS1024W: 4}
 
 
@@ -252,12 +268,13 @@ def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, 
     if job.bound == "hbm":
         ach = job.alg_per_launch() / sec_per_launch / 1e9
         res["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                           "frac": ach / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"] + " copy bandwidth"}
+                           "frac": ach / peaks["hbm_gbs"], "traffic": measured_traffic(job.name),
+                           "algorithmic_bytes": job.alg_per_launch(), "peak_source": peaks["source"] + " copy bandwidth"}
     else:
         ach = job.alg_per_launch() / sec_per_launch / 1e12
         peak = issue_peak_tinst(peaks["sm_max_mhz"])
         res["roofline"] = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tinst/s", "frac": ach / peak,
-                           "traffic": None,
+                           "traffic": measured_traffic(job.name),
                            "peak_source": "148 SM x 4 SMSP x 32 lanes x sm_max_mhz (issue slots; DESIGN.md s7)"}
     if clocks:
         res["clocks"] = clocks
