@@ -45,6 +45,8 @@ def lib():
         L.orc_splitmix64.argtypes = [u64, u64]
         L.orc_lcg64_step.restype = u64
         L.orc_lcg64_step.argtypes = [u64]
+        L.orc_lcg32_step.restype = u32
+        L.orc_lcg32_step.argtypes = [u32]
         L.orc_lcg64_jump.restype = None
         L.orc_lcg64_jump.argtypes = [u64, C.POINTER(u64), C.POINTER(u64)]
         L.orc_philox4x32.restype = None
@@ -94,6 +96,10 @@ def splitmix64(seed: int, k: int) -> int:
 
 def lcg64_step(x: int) -> int:
     return int(lib().orc_lcg64_step(x))
+
+
+def lcg32_step(x: int) -> int:
+    return int(lib().orc_lcg32_step(x))
 
 
 def lcg64_jump(n: int):

@@ -177,12 +177,16 @@ struct orc_rng {
     uint64_t leap_X;      /* LEAPFROG: X_{draws_done * n_total} of the global sequence */
     uint32_t *xw;         /* XORWOW: [n_local][6] */
     uint32_t *xs;         /* XS1024W: [n_local/32][32], word i of instance g at 32 g + i */
+    uint32_t *lcg32;      /* LCG32: x of each local stream */
 };
+
+/* G1: 32-bit LCG, eq.(1) with the constants of PAPER.md:46 */
+uint32_t orc_lcg32_step(uint32_t x) { return 1664525u * x + 1013904223u; }
 
 orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local, uint64_t seed)
 {
     if (n_local < 1 || first + n_local > n_total || first + n_local < first) return NULL;
-    if (kind < ORC_LCG64 || kind > ORC_XS1024W) return NULL;
+    if (kind < ORC_LCG64 || kind > ORC_LCG32) return NULL;
     if (kind == ORC_XS1024W && (first % 32 || n_local % 32)) return NULL;
     orc_rng *r = (orc_rng *)calloc(1, sizeof *r);
     if (!r) return NULL;
@@ -208,6 +212,11 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
         }
         break;
     case ORC_PHILOX4X32_10: /* no state: key and counter are intrinsic */
+    case ORC_PHILOX4X32_7:
+        break;
+    case ORC_LCG32: /* random seeding */
+        r->lcg32 = (uint32_t *)malloc(n_local * sizeof(uint32_t));
+        for (uint64_t s = 0; s < n_local; s++) r->lcg32[s] = (uint32_t)orc_splitmix64(seed, first + s);
         break;
     case ORC_XS1024W: /* "sloppy" random seeding; R-D7 */
         r->xs = (uint32_t *)malloc(n_local * sizeof(uint32_t));
@@ -230,7 +239,7 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
 void orc_destroy(orc_rng *r)
 {
     if (!r) return;
-    free(r->lcg); free(r->xw); free(r->xs); free(r);
+    free(r->lcg); free(r->xw); free(r->xs); free(r->lcg32); free(r);
 }
 
 uint64_t orc_draws_done(const orc_rng *r) { return r->draws_done; }
@@ -238,13 +247,13 @@ uint64_t orc_draws_done(const orc_rng *r) { return r->draws_done; }
 /* Philox stream mapping (BASELINE.json config 2, R-C2): key = stream id XOR
  * seed (64 bit, k0 = low word); counter = index of the 4-word block,
  * (lo32(b), hi32(b), 0, 0); draw j is word (j mod 4) of block floor(j/4). */
-static uint32_t philox_draw(uint64_t stream_id, uint64_t seed, uint64_t j)
+static uint32_t philox_draw(int rounds, uint64_t stream_id, uint64_t seed, uint64_t j)
 {
     uint64_t K = stream_id ^ seed, b = j / 4;
     uint32_t key[2] = {(uint32_t)K, (uint32_t)(K >> 32)};
     uint32_t ctr[4] = {(uint32_t)b, (uint32_t)(b >> 32), 0u, 0u};
     uint32_t o[4];
-    orc_philox4x32(10, ctr, key, o);
+    orc_philox4x32(rounds, ctr, key, o);
     return o[j % 4];
 }
 
@@ -283,10 +292,24 @@ void orc_fill_u32(orc_rng *r, uint32_t *out, uint64_t n)
             for (uint64_t j = 0; j < n; j++) out[s * n + j] = orc_xorwow_next(r->xw + 6 * s);
         break;
     case ORC_PHILOX4X32_10:
+    case ORC_PHILOX4X32_7: {
+        const int rounds = r->kind == ORC_PHILOX4X32_7 ? 7 : 10;
 #pragma omp parallel for schedule(static)
         for (uint64_t s = 0; s < S; s++)
             for (uint64_t j = 0; j < n; j++)
-                out[s * n + j] = philox_draw(r->first + s, r->seed, r->draws_done + j);
+                out[s * n + j] = philox_draw(rounds, r->first + s, r->seed, r->draws_done + j);
+        break;
+    }
+    case ORC_LCG32:
+#pragma omp parallel for schedule(static)
+        for (uint64_t s = 0; s < S; s++) {
+            uint32_t x = r->lcg32[s];
+            for (uint64_t j = 0; j < n; j++) {
+                out[s * n + j] = x; /* u_n = x_n / m: the whole word is the output */
+                x = orc_lcg32_step(x);
+            }
+            r->lcg32[s] = x;
+        }
         break;
     case ORC_XS1024W:
         /* stream s = word (s mod 32) of instance floor(s/32)  (R-D4) */
@@ -341,6 +364,7 @@ uint64_t orc_state_words32(const orc_rng *r)
     case ORC_LCG64: case ORC_LCG64_LEAPFROG: return 2 * r->n_local;
     case ORC_XORWOW: return 6 * r->n_local;
     case ORC_XS1024W: return r->n_local;
+    case ORC_LCG32: return r->n_local;
     default: return 0;
     }
 }
@@ -359,6 +383,7 @@ void orc_get_state(const orc_rng *r, uint32_t *out)
     }
     case ORC_XORWOW: memcpy(out, r->xw, r->n_local * 24); break;
     case ORC_XS1024W: memcpy(out, r->xs, r->n_local * 4); break;
+    case ORC_LCG32: memcpy(out, r->lcg32, r->n_local * 4); break;
     default: break;
     }
 }

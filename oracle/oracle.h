@@ -32,7 +32,10 @@ enum {
     ORC_LCG64_LEAPFROG = 1, /* PAPER.md:39-46 eq.(2),(3): one global sequence   */
     ORC_XORWOW         = 2, /* PAPER.md:169, :236 (recurrence: Ref.[30], R-B1)  */
     ORC_PHILOX4X32_10  = 3, /* PAPER.md:284-296 (constants: Ref.[20], R-C1)     */
-    ORC_XS1024W        = 4  /* PAPER.md:166 eq.(8), :177, :201-225, :232-240    */
+    ORC_XS1024W        = 4, /* PAPER.md:166 eq.(8), :177, :201-225, :232-240    */
+    ORC_PHILOX4X32_7   = 5, /* the 7-round variant          */
+    ORC_LCG32          = 6  /* PAPER.md:33 eq.(1), :46: a=1664525, c=1013904223,
+                               m=2^32; draw j = x_j (all 32 bits), x_0 = lo32(SM_seed[s]) */
 };
 
 /* ---- elementary pieces, exported so that the tests can pin them ---------- */
@@ -42,6 +45,7 @@ uint64_t orc_splitmix64(uint64_t seed, uint64_t k);
 
 /* one step of eq.(1) with m = 2^64 */
 uint64_t orc_lcg64_step(uint64_t x);
+uint32_t orc_lcg32_step(uint32_t x);
 
 /* eq.(2): the affine map x -> A x + C equal to n steps of eq.(1), evaluated by
  * the CLOSED FORM  A = a^n,  C = c (a^n - 1)/(a - 1)  (mod 2^64)  in 128-bit
