@@ -68,11 +68,13 @@ def issue_peak_tinst(sm_mhz: float) -> float:
 # Philox = per word 5 mulhi/lo + 5 xors + key/counter (2); xs1024 register-resident = 66 funnel
 # shifts + 66 xors per 32 words (the zero padding drops 10 of 32 words per phase) + Weyl add (1)
 # + checksum (2)
-ALG_INST_PER_DRAW = {W.LCG64: 5.0, W.LCG64_LEAPFROG: 5.0, W.XORWOW: 10.0, W.PHILOX4X32_10: 12.0, W.XS1024W: 7.0}
+ALG_INST_PER_DRAW = {W.LCG64: 5.0, W.LCG64_LEAPFROG: 5.0, W.XORWOW: 10.0, W.PHILOX4X32_10: 12.0, W.XS1024W: 7.0,
+                     W.PHILOX4X32_7: 9.0, W.LCG32: 3.0}
 # multi-spin-coded update: two threshold compares of two instructions each + the bit-sliced
 # neighbour count / flip logic amortised over the 32 sites of a word (about 1), excl. the draw
 ALG_INST_PER_ISING_UPDATE = 5.0
-STATE_BYTES = {W.LCG64: 8, W.LCG64_LEAPFROG: 8, W.XORWOW: 24, W.PHILOX4X32_10: 0, W.XS1024W: 4}
+STATE_BYTES = {W.LCG64: 8, W.LCG64_LEAPFROG: 8, W.XORWOW: 24, W.PHILOX4X32_10: 0, W.XS1024W: 4, W.PHILOX4X32_7: 0,
+               W.LCG32: 4}
 
 
 class ClockSampler:
@@ -292,6 +294,12 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
         "C1_f32": lambda: FillJob(W.C1, True, rank, world, buf),
         "C1big_u32": lambda: FillJob(W.C1_BIG, False, rank, world, buf),
         "C3fill_u32": lambda: FillJob(W.C3_FILL, False, rank, world, buf),
+        "N1_philox7_u32": lambda: FillJob(W.N1_PHILOX7, False, rank, world, buf),
+        "N1_lcg32_u32": lambda: FillJob(W.N1_LCG32, False, rank, world, buf),
+        "N1_philox7_draw": lambda: DrawJob(W.N1_PHILOX7_DRAW, rank, world, buf),
+        "N1_philox10_draw": lambda: DrawJob(W.N1_PHILOX10_DRAW, rank, world, buf),
+        "N1_lcg32_draw": lambda: DrawJob(W.N1_LCG32_DRAW, rank, world, buf),
+        "N1_lcg64_draw": lambda: DrawJob(W.N1_LCG64_DRAW, rank, world, buf),
         "C3_draw": lambda: DrawJob(W.C3, rank, world, buf),
         "C4_fill": lambda: FillJob(W.C4_FILL, False, rank, world, buf),
         "C4_draw": lambda: DrawJob(W.C4_DRAW, rank, world, buf),
@@ -308,7 +316,9 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
 # default run stays within a few minutes
 SUITE = [("C2_f32", 20, 3), ("C1_u32", 200, 10), ("C1_f32", 200, 10), ("C1big_u32", 20, 3), ("C3fill_u32", 20, 3),
          ("C3_draw", 20, 3), ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1),
-         ("C5b_xorwow_K8", 1, 1)]
+         ("C5b_xorwow_K8", 1, 1),
+         ("N1_philox7_u32", 20, 3), ("N1_lcg32_u32", 20, 3), ("N1_philox7_draw", 20, 3), ("N1_philox10_draw", 20, 3),
+         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3)]
 
 
 # ------------------------------------------------------------------------------------
@@ -337,7 +347,10 @@ def oracle_sample_rate(workload: str, target_s: float = 4.0) -> dict:
                 "sample": f"L={L} (1/16 of the 8192^2 lattice, same sites per stream), {sweeps} sweeps", "seconds": dt}
     cfgs = {"C2_u32": (W.C2, "fill_u32"), "C2_f32": (W.C2, "fill_f32"), "C1_u32": (W.C1, "fill_u32"),
             "C1_f32": (W.C1, "fill_f32"), "C1big_u32": (W.C1_BIG, "fill_u32"), "C3fill_u32": (W.C3_FILL, "fill_u32"),
-            "C3_draw": (W.C3, "draw_reduce"), "C4_fill": (W.C4_FILL, "fill_u32"), "C4_draw": (W.C4_DRAW, "draw_reduce")}
+            "C3_draw": (W.C3, "draw_reduce"), "C4_fill": (W.C4_FILL, "fill_u32"), "C4_draw": (W.C4_DRAW, "draw_reduce"),
+            "N1_philox7_u32": (W.N1_PHILOX7, "fill_u32"), "N1_lcg32_u32": (W.N1_LCG32, "fill_u32"),
+            "N1_philox7_draw": (W.N1_PHILOX7_DRAW, "draw_reduce"), "N1_philox10_draw": (W.N1_PHILOX10_DRAW, "draw_reduce"),
+            "N1_lcg32_draw": (W.N1_LCG32_DRAW, "draw_reduce"), "N1_lcg64_draw": (W.N1_LCG64_DRAW, "draw_reduce")}
     cfg, call = cfgs[workload]
     n = cfg.n_per_stream
     # calibrate on a small slice of the streams, then time one slice of about target_s

@@ -77,7 +77,15 @@ enum {
      * R-D7): words 2k, 2k+1 of instance g = lo32, hi32 of SM_seed[16g+k]; an
      * all-zero instance gets word 31 = 1.  n_streams and first must be
      * multiples of 32. */
-    RNG_XS1024W = 4
+    RNG_XS1024W = 4,
+    /* Philox4x32 with 7 rounds (PAPER.md:269 Table 2, :300: "the fastest Crush-resistant"
+     * variant; same S-box, constants, key schedule and stream mapping as kind 3). */
+    RNG_PHILOX4X32_7 = 5,
+    /* the 32-bit LCG of PAPER.md:33 eq.(1) with a = 1664525, c = 1013904223, m = 2^32
+     * (Table 2 "LCG32"): draw j = x_j, the whole word (u = x/m, PAPER.md:35;
+     * output, then advance); x_0 of stream s = lo32(SM_seed[s]).  Period 2^32: the paper's
+     * deliberately bad example (fails SmallCrush), here for its Table-2 row. */
+    RNG_LCG32 = 6
 };
 
 enum {
@@ -162,7 +170,8 @@ int ising_sweep_host(rng_handle *h, int8_t *h_spins, uint32_t L, double beta, ui
  * Canonical order, independent of the device layout:
  *   LCG64 / LEAPFROG: n_local x u64 (current x of each stream)
  *   XORWOW: n_local x {x,y,z,w,v,d} u32, stream-major
- *   PHILOX: 0 bytes;  XS1024W: n_local x u32 (word s%32 of instance s/32)
+ *   PHILOX (both): 0 bytes;  XS1024W: n_local x u32 (word s%32 of instance s/32)
+ *   LCG32: n_local x u32 (current x of each stream)
  * rng_get_state/rng_set_state synchronise the device; bytes must equal
  * rng_state_bytes(kind, n_local).  draws_done is read / set separately. */
 uint64_t rng_state_bytes(int kind, uint64_t n_streams);

@@ -48,6 +48,7 @@ __global__ void __launch_bounds__(256) draw_reduce_kernel(Gen g, uint2 *__restri
 
 // Philox: counter-based, so the n draws of a stream are the words of consecutive blocks;
 // whole blocks are reduced four words at a time with the round keys' base hoisted.
+template <int R>
 __global__ void __launch_bounds__(256) philox_draw_reduce_kernel(Gen g, uint2 *__restrict__ out, uint64_t n)
 {
     const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -60,7 +61,7 @@ __global__ void __launch_bounds__(256) philox_draw_reduce_kernel(Gen g, uint2 *_
     // head: words of a partially consumed block
     if ((j & 3ull) && j < end) {
         const uint64_t b = j >> 2;
-        const uint4 r = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+        const uint4 r = philox4x32<R>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
         const uint32_t w[4] = {r.x, r.y, r.z, r.w};
         for (; (j & 3ull) && j < end; j++) {
             x ^= w[j & 3ull];
@@ -69,13 +70,13 @@ __global__ void __launch_bounds__(256) philox_draw_reduce_kernel(Gen g, uint2 *_
     }
     for (; j + 4 <= end; j += 4) {
         const uint64_t b = j >> 2;
-        const uint4 r = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+        const uint4 r = philox4x32<R>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
         x ^= r.x ^ r.y ^ r.z ^ r.w;
         sum += r.x + r.y + r.z + r.w;
     }
     if (j < end) { // tail
         const uint64_t b = j >> 2;
-        const uint4 r = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+        const uint4 r = philox4x32<R>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
         const uint32_t w[4] = {r.x, r.y, r.z, r.w};
         for (; j < end; j++) {
             x ^= w[j & 3ull];
@@ -97,7 +98,9 @@ cudaError_t launch_draw_reduce(const rng_handle &h, uint32_t *d_out, uint64_t n,
     case RNG_LCG64_LEAPFROG: draw_reduce_kernel<RNG_LCG64_LEAPFROG><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     case RNG_XORWOW: draw_reduce_kernel<RNG_XORWOW><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     case RNG_XS1024W: draw_reduce_kernel<RNG_XS1024W><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
-    case RNG_PHILOX4X32_10: philox_draw_reduce_kernel<<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_PHILOX4X32_10: philox_draw_reduce_kernel<10><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_PHILOX4X32_7: philox_draw_reduce_kernel<7><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_LCG32: draw_reduce_kernel<RNG_LCG32><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     default: return cudaErrorInvalidValue;
     }
     count_launch();

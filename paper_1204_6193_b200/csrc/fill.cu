@@ -19,7 +19,7 @@ namespace rngb200 {
 // row; tiles are handed to CTAs grid-stride.  ALIGNED (d0 % 4 == 0 and n % 4 == 0): every
 // block is written whole with a 128-bit store; otherwise word by word with bounds checks.
 // ------------------------------------------------------------------------------------
-template <bool F32, bool ALIGNED, int U>
+template <bool F32, bool ALIGNED, int U, int R>
 __global__ void __launch_bounds__(256) philox_fill_kernel(uint32_t *__restrict__ out, uint64_t S, uint64_t first,
                                                          uint64_t seed, uint64_t d0, uint64_t n,
                                                          uint64_t blocks_per_row, uint32_t tiles_per_row,
@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(256) philox_fill_kernel(uint32_t *__restrict__
             const uint64_t rb = (uint64_t)c * (256 * U) + u * 256 + threadIdx.x; // block within the row
             if (rb >= blocks_per_row) continue;
             const uint64_t b = b0 + rb; // counter = index of the 4-word block
-            uint4 r = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+            uint4 r = philox4x32<R>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
             r.x = out_word(r.x, F32);
             r.y = out_word(r.y, F32);
             r.z = out_word(r.z, F32);
@@ -74,10 +74,10 @@ __global__ void __launch_bounds__(256) philox_fill_kernel(uint32_t *__restrict__
 // ------------------------------------------------------------------------------------
 // U independent 4-word blocks per lane (blocks rb0, rb0+32, ...), ten rounds interleaved,
 // one 128-bit streaming store each.  CHECK = bounds-check each block (ragged last tile).
-template <bool F32, int U, bool CHECK>
+template <bool F32, int U, bool CHECK, int R>
 __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_t b0, uint32_t rb0,
-                                             uint32_t blocks_per_row, const uint32_t (&rk0)[10],
-                                             const uint32_t (&rk1)[10])
+                                             uint32_t blocks_per_row, const uint32_t (&rk0)[R],
+                                             const uint32_t (&rk1)[R])
 {
     uint32_t c0[U], c1[U], c2[U], c3[U];
 #pragma unroll
@@ -89,7 +89,7 @@ __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_
         c3[u] = 0u;
     }
 #pragma unroll
-    for (int r = 0; r < 10; r++) {
+    for (int r = 0; r < R; r++) {
 #pragma unroll
         for (int u = 0; u < U; u++) {
             const uint64_t p0 = (uint64_t)kPhM0 * c0[u];
@@ -113,7 +113,7 @@ __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_
     }
 }
 
-template <bool F32, int U, int T>
+template <bool F32, int U, int T, int R>
 __global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restrict__ out, uint64_t first, uint64_t seed,
                                                               uint64_t b0, uint64_t n, uint32_t blocks_per_row,
                                                               uint32_t tiles_per_row, uint64_t n_tiles)
@@ -129,9 +129,9 @@ __global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restr
     const uint32_t dc = (uint32_t)(n_warps - ds * tiles_per_row);
     for (; t < n_tiles; t += n_warps) {
         const uint64_t key = (first + s) ^ seed; // R-C2: key = stream id ^ seed
-        uint32_t rk0[10], rk1[10];
+        uint32_t rk0[R], rk1[R];
 #pragma unroll
-        for (int r = 0; r < 10; r++) {
+        for (int r = 0; r < R; r++) {
             rk0[r] = (uint32_t)key + (uint32_t)r * kPhW0;
             rk1[r] = (uint32_t)(key >> 32) + (uint32_t)r * kPhW1;
         }
@@ -140,11 +140,11 @@ __global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restr
         if (tile_full) {
 #pragma unroll 1
             for (int g = 0; g < T; g++)
-                philox_group<F32, U, false>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
+                philox_group<F32, U, false, R>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
         } else {
 #pragma unroll 1
             for (int g = 0; g < T; g++)
-                philox_group<F32, U, true>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
+                philox_group<F32, U, true, R>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
         }
         s += ds;
         c += dc;
@@ -326,7 +326,7 @@ static cudaError_t launch_rowtile(const Gen &g, void *d_out, uint64_t n, bool f3
     return cudaGetLastError();
 }
 
-template <bool F32, int U, int T>
+template <bool F32, int U, int T, int R>
 static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uint64_t blocks_per_row, cudaStream_t st)
 {
     const uint64_t tpr = (blocks_per_row + 32 * U * T - 1) / (32 * U * T);
@@ -335,19 +335,20 @@ static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uin
     static int per_sm = 0;
     if (!per_sm) {
         int b = 0;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, philox_fill_warp_kernel<F32, U, T>, 256, 0);
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, philox_fill_warp_kernel<F32, U, T, R>, 256, 0);
         if (e != cudaSuccess) return e;
         per_sm = b > 0 ? b : 1;
     }
     uint64_t grid = (uint64_t)sm_count() * per_sm;
     const uint64_t need = (n_tiles + 7) / 8;
     if (grid > need) grid = need;
-    philox_fill_warp_kernel<F32, U, T><<<(unsigned)grid, 256, 0, st>>>(o, g.first, g.seed, g.draws_done >> 2, n,
+    philox_fill_warp_kernel<F32, U, T, R><<<(unsigned)grid, 256, 0, st>>>(o, g.first, g.seed, g.draws_done >> 2, n,
                                                                      (uint32_t)blocks_per_row, (uint32_t)tpr, n_tiles);
     count_launch();
     return cudaGetLastError();
 }
 
+template <int R>
 static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, bool f32, int variant, cudaStream_t st)
 {
     const uint64_t d0 = g.draws_done;
@@ -355,8 +356,8 @@ static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, boo
     const bool aligned = ((d0 | n) & 3ull) == 0ull;
     uint32_t *o = (uint32_t *)d_out;
     if (aligned && blocks_per_row <= 0x7fffffffull) {
-#define PW(U, T) (f32 ? launch_philox_warp<true, U, T>(g, o, n, blocks_per_row, st) \
-                      : launch_philox_warp<false, U, T>(g, o, n, blocks_per_row, st))
+#define PW(U, T) (f32 ? launch_philox_warp<true, U, T, R>(g, o, n, blocks_per_row, st) \
+                      : launch_philox_warp<false, U, T, R>(g, o, n, blocks_per_row, st))
         switch (variant) { // identical bits; (U, T) = blocks interleaved per lane, groups per tile
         case 1: return PW(4, 2);
         case 2: return PW(2, 4);
@@ -372,10 +373,10 @@ static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, boo
     uint64_t grid = (uint64_t)sm_count() * 8ull;
     if (grid > n_tiles) grid = n_tiles;
     if (f32)
-        philox_fill_kernel<true, false, U><<<(unsigned)grid, 256, 0, st>>>(o, g.S, g.first, g.seed, d0, n, blocks_per_row,
+        philox_fill_kernel<true, false, U, R><<<(unsigned)grid, 256, 0, st>>>(o, g.S, g.first, g.seed, d0, n, blocks_per_row,
                                                                           (uint32_t)tpr, n_tiles);
     else
-        philox_fill_kernel<false, false, U><<<(unsigned)grid, 256, 0, st>>>(o, g.S, g.first, g.seed, d0, n, blocks_per_row,
+        philox_fill_kernel<false, false, U, R><<<(unsigned)grid, 256, 0, st>>>(o, g.S, g.first, g.seed, d0, n, blocks_per_row,
                                                                            (uint32_t)tpr, n_tiles);
     count_launch();
     return cudaGetLastError();
@@ -396,7 +397,9 @@ cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, 
     case RNG_XS1024W:
         if (h.var_xs1024 == 64) return launch_rowtile<RNG_XS1024W>(g, d_out, n, f32, h.var_store, st);
         return launch_xs1024_fill(h, d_out, n, f32, st);
-    case RNG_PHILOX4X32_10: return launch_philox_fill(g, d_out, n, f32, h.var_store, st);
+    case RNG_PHILOX4X32_10: return launch_philox_fill<10>(g, d_out, n, f32, h.var_store, st);
+    case RNG_PHILOX4X32_7: return launch_philox_fill<7>(g, d_out, n, f32, h.var_store, st);
+    case RNG_LCG32: return launch_rowtile<RNG_LCG32>(g, d_out, n, f32, h.var_store, st);
     default: return cudaErrorInvalidValue;
     }
 }

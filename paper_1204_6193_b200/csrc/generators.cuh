@@ -6,6 +6,8 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#include "../../include/rng_b200.h"
+
 namespace rngb200 {
 
 // ---------------------------------------------------------------------------------
@@ -29,6 +31,9 @@ struct Affine {
 };
 constexpr uint64_t kLcgA = 2862933555777941757ull;
 constexpr uint64_t kLcgC = 1442695040888963407ull;
+// the 32-bit LCG of PAPER.md:46 (a = 1664525, c = 1013904223, m = 2^32; Table 2 "LCG32")
+constexpr uint32_t kLcg32A = 1664525u;
+constexpr uint32_t kLcg32C = 1013904223u;
 
 __host__ __device__ __forceinline__ uint64_t affine_apply(const Affine &m, uint64_t x) { return m.A * x + m.C; }
 // f after g:  f(g(x)) = (A_f A_g) x + (A_f C_g + C_f)
@@ -88,6 +93,11 @@ struct Xorwow {
 // ---------------------------------------------------------------------------------
 constexpr uint32_t kPhM0 = 0xD2511F53u, kPhM1 = 0xCD9E8D57u;
 constexpr uint32_t kPhW0 = 0x9E3779B9u, kPhW1 = 0xBB67AE85u;
+
+// kinds that are Philox4x32-R (counter-based, stateless) and their number of rounds
+// (the 7-round variant is the paper's fastest Crush-resistant choice)
+__host__ __device__ constexpr bool kind_is_philox(int kind) { return kind == RNG_PHILOX4X32_10 || kind == RNG_PHILOX4X32_7; }
+__host__ __device__ constexpr int philox_rounds(int kind) { return kind == RNG_PHILOX4X32_7 ? 7 : 10; }
 
 template <int R = 10>
 __device__ __forceinline__ uint4 philox4x32(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,

@@ -23,6 +23,7 @@ struct LcgTable {
 //   XORWOW           : u32 w[6][S]   (word k of stream s at w[k*S + s]; k = x,y,z,w,v,d)
 //   PHILOX           : none
 //   XS1024W          : u32 w[S]      (word `lane` of instance g at w[32 g + lane])
+//   LCG32            : u32 x[S]
 struct Gen {
     int kind;
     uint64_t S;          // local streams
@@ -50,6 +51,19 @@ struct rng_handle {
     uint64_t ms_planes_bytes;
     int var_xs1024, var_ising, var_store, var_lcg;
 };
+
+// run MACRO(KIND) for the runtime kind (every kind that has a Stream<KIND>)
+#define RNGB200_DISPATCH_KIND(kind, MACRO)                          \
+    switch (kind) {                                                 \
+    case RNG_LCG64: MACRO(RNG_LCG64); break;                        \
+    case RNG_LCG64_LEAPFROG: MACRO(RNG_LCG64_LEAPFROG); break;      \
+    case RNG_XORWOW: MACRO(RNG_XORWOW); break;                      \
+    case RNG_PHILOX4X32_10: MACRO(RNG_PHILOX4X32_10); break;        \
+    case RNG_XS1024W: MACRO(RNG_XS1024W); break;                    \
+    case RNG_PHILOX4X32_7: MACRO(RNG_PHILOX4X32_7); break;          \
+    case RNG_LCG32: MACRO(RNG_LCG32); break;                        \
+    default: return cudaErrorInvalidValue;                          \
+    }
 
 namespace rngb200 {
 

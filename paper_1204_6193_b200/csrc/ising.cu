@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(256) ising_chunk_kernel(Gen g, int8_t *__restr
 
     // the 8 draws of this chunk, in site order
     uint32_t rnd[8];
-    if (KIND == RNG_PHILOX4X32_10) {
+    if (kind_is_philox(KIND)) {
         const uint64_t q0 = (uint64_t)y * (L >> 1) + 8ull * cx;
 #pragma unroll
         for (int gi = 0; gi < 2; gi++) {
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(256) ising_chunk_kernel(Gen g, int8_t *__restr
             const uint64_t k = qg - s * K;
             const uint64_t key = (g.first + s) ^ g.seed;
             const uint64_t b = (g.draws_done + k) >> 2;
-            const uint4 o = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, (uint32_t)key, (uint32_t)(key >> 32));
+            const uint4 o = philox4x32<philox_rounds(KIND)>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, (uint32_t)key, (uint32_t)(key >> 32));
             rnd[4 * gi + 0] = o.x;
             rnd[4 * gi + 1] = o.y;
             rnd[4 * gi + 2] = o.z;
@@ -229,7 +229,7 @@ cudaError_t launch_ising_half_sweep(const rng_handle &h, int8_t *d_spins, uint32
         const uint32_t cpr = L >> 4;
         const bool geom_ok = (L % 16u) == 0u && L >= 16u && L <= 65536u && h.var_ising != 1;
         bool kind_ok;
-        if (g.kind == RNG_PHILOX4X32_10) kind_ok = (K % 4ull) == 0ull && (draws_done % 4ull) == 0ull;
+        if (kind_is_philox(g.kind)) kind_ok = (K % 4ull) == 0ull && (draws_done % 4ull) == 0ull;
         else if (g.kind == RNG_XS1024W) kind_ok = K == 8ull && (cpr % 32u) == 0u;
         else kind_ok = K == 8ull;
         if (thr_ok && geom_ok && kind_ok) {
@@ -240,14 +240,7 @@ cudaError_t launch_ising_half_sweep(const rng_handle &h, int8_t *d_spins, uint32
             }
             const dim3 blk(32, 8), grd((cpr + 31) / 32, L / 8);
 #define CHUNK(KIND) ising_chunk_kernel<KIND><<<grd, blk, 0, st>>>(g, d_spins, L, ft, (uint32_t)K, log2K, colour)
-            switch (g.kind) {
-            case RNG_LCG64: CHUNK(RNG_LCG64); break;
-            case RNG_LCG64_LEAPFROG: CHUNK(RNG_LCG64_LEAPFROG); break;
-            case RNG_XORWOW: CHUNK(RNG_XORWOW); break;
-            case RNG_XS1024W: CHUNK(RNG_XS1024W); break;
-            case RNG_PHILOX4X32_10: CHUNK(RNG_PHILOX4X32_10); break;
-            default: return cudaErrorInvalidValue;
-            }
+            RNGB200_DISPATCH_KIND(g.kind, CHUNK)
 #undef CHUNK
             count_launch();
             return cudaGetLastError();
@@ -257,14 +250,7 @@ cudaError_t launch_ising_half_sweep(const rng_handle &h, int8_t *d_spins, uint32
     if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
 #define GENERIC(KIND) \
     ising_half_sweep_generic_kernel<KIND><<<(unsigned)grid, 256, 0, st>>>(g, d_spins, L, tab, K, colour)
-    switch (g.kind) {
-    case RNG_LCG64: GENERIC(RNG_LCG64); break;
-    case RNG_LCG64_LEAPFROG: GENERIC(RNG_LCG64_LEAPFROG); break;
-    case RNG_XORWOW: GENERIC(RNG_XORWOW); break;
-    case RNG_XS1024W: GENERIC(RNG_XS1024W); break;
-    case RNG_PHILOX4X32_10: GENERIC(RNG_PHILOX4X32_10); break;
-    default: return cudaErrorInvalidValue;
-    }
+    RNGB200_DISPATCH_KIND(g.kind, GENERIC)
 #undef GENERIC
     count_launch();
     return cudaGetLastError();

@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(64) ising_ms_stream_kernel(Gen g, uint32_t *__
     const uint32_t wpr = L >> 6;
     uint32_t widx = (uint32_t)s * W;
     uint32_t y = widx / wpr, j = widx - y * wpr;
-    if (KIND == RNG_PHILOX4X32_10) {
+    if (kind_is_philox(KIND)) {
         const uint64_t key = (g.first + s) ^ g.seed;
         const uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
         uint64_t b = g.draws_done >> 2; // draws_done % 4 == 0 (host-checked): whole blocks
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(64) ising_ms_stream_kernel(Gen g, uint32_t *__
             uint32_t n0 = 0u, n1 = 0u;
 #pragma unroll
             for (int gi = 0; gi < 8; gi++, b++) {
-                const uint4 o = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+                const uint4 o = philox4x32<philox_rounds(KIND)>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
                 ms_cmp_insert(o.x, thr, n0, n1);
                 ms_cmp_insert(o.y, thr, n0, n1);
                 ms_cmp_insert(o.z, thr, n0, n1);
@@ -188,14 +188,14 @@ __global__ void __launch_bounds__(128) ising_ms_word_kernel(Gen g, uint32_t *__r
     mw.load(Cp, Np, L, wpr, y, j, colour);
     uint32_t n0 = 0u, n1 = 0u;
     const uint64_t s0 = (uint64_t)widx * (32 / K);
-    if (KIND == RNG_PHILOX4X32_10) {
+    if (kind_is_philox(KIND)) {
         const uint64_t b0 = g.draws_done >> 2; // draws_done % 4 == 0
 #pragma unroll
         for (int gi = 0; gi < 8; gi++) {
             const uint64_t s = s0 + (4 * gi) / K;
             const uint64_t b = b0 + ((4 * gi) % K) / 4;
             const uint64_t key = (g.first + s) ^ g.seed;
-            const uint4 o = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, (uint32_t)key, (uint32_t)(key >> 32));
+            const uint4 o = philox4x32<philox_rounds(KIND)>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, (uint32_t)key, (uint32_t)(key >> 32));
             ms_cmp_insert(o.x, thr, n0, n1);
             ms_cmp_insert(o.y, thr, n0, n1);
             ms_cmp_insert(o.z, thr, n0, n1);
@@ -323,7 +323,7 @@ bool ising_ms_eligible(const rng_handle &h, uint32_t L, const IsingTable &tab, u
     if (tab.T[0] != one || tab.T[1] != one || tab.T[2] != one) return false;
     if (tab.T[4] < 1u || tab.T[4] > tab.T[3] || tab.T[3] > one) return false;
     const int kind = h.g.kind;
-    if (kind == RNG_PHILOX4X32_10 && (draws_done & 3ull)) return false;
+    if (kind_is_philox(kind) && (draws_done & 3ull)) return false;
     if (K % 32ull == 0ull) return K / 32ull <= 0xffffffffull && h.g.S <= 0x7fffffffull;
     if (K == 4 || K == 8 || K == 16) return kind != RNG_XS1024W;
     return false;
@@ -384,14 +384,7 @@ cudaError_t launch_ising_ms_half_sweep(const rng_handle &h, uint32_t *planes, ui
         const uint32_t W = (uint32_t)(K / 32ull);
         const uint32_t grid = (uint32_t)((g.S + 63) / 64);
 #define MS_STREAM(KIND) ising_ms_stream_kernel<KIND><<<grid, 64, 0, st>>>(g, Cp, Np, L, thr, W, (uint32_t)colour)
-        switch (g.kind) {
-        case RNG_LCG64: MS_STREAM(RNG_LCG64); break;
-        case RNG_LCG64_LEAPFROG: MS_STREAM(RNG_LCG64_LEAPFROG); break;
-        case RNG_XORWOW: MS_STREAM(RNG_XORWOW); break;
-        case RNG_XS1024W: MS_STREAM(RNG_XS1024W); break;
-        case RNG_PHILOX4X32_10: MS_STREAM(RNG_PHILOX4X32_10); break;
-        default: return cudaErrorInvalidValue;
-        }
+        RNGB200_DISPATCH_KIND(g.kind, MS_STREAM)
 #undef MS_STREAM
     } else {
         switch (g.kind) {
@@ -399,6 +392,8 @@ cudaError_t launch_ising_ms_half_sweep(const rng_handle &h, uint32_t *planes, ui
         case RNG_LCG64_LEAPFROG: launch_ms_word<RNG_LCG64_LEAPFROG>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         case RNG_XORWOW: launch_ms_word<RNG_XORWOW>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         case RNG_PHILOX4X32_10: launch_ms_word<RNG_PHILOX4X32_10>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
+        case RNG_PHILOX4X32_7: launch_ms_word<RNG_PHILOX4X32_7>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
+        case RNG_LCG32: launch_ms_word<RNG_LCG32>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         default: return cudaErrorInvalidValue;
         }
     }

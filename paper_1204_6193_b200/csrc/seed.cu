@@ -39,6 +39,13 @@ __global__ void seed_lcg64_kernel(uint64_t *x, uint64_t S, uint64_t first, uint6
     if (s < S) x[s] = splitmix64_at(seed, first + s);
 }
 
+// RNG_LCG32: x_0 of stream s = lo32(SM_seed[s])
+__global__ void seed_lcg32_kernel(uint32_t *x, uint64_t S, uint64_t first, uint64_t seed)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < S) x[s] = (uint32_t)splitmix64_at(seed, first + s);
+}
+
 // RNG_LCG64_LEAPFROG: one global sequence X_0 = SM_seed[0]; stream s starts at X_s =
 // (a,c)^s applied to X_0 -- eq.(2) with t = s, by binary exponentiation.
 __global__ void seed_lcg64_leapfrog_kernel(uint64_t *x, uint64_t S, uint64_t first, uint64_t seed)
@@ -108,7 +115,12 @@ cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st)
         seed_xs1024_kernel<<<grid, B, 0, st>>>((uint32_t *)g.state, g.S, g.first, g.seed);
         count_launch();
         break;
+    case RNG_LCG32:
+        seed_lcg32_kernel<<<grid, B, 0, st>>>((uint32_t *)g.state, g.S, g.first, g.seed);
+        count_launch();
+        break;
     case RNG_PHILOX4X32_10:
+    case RNG_PHILOX4X32_7:
     default:
         break; // key = s ^ seed and counter = draw index are intrinsic: nothing to set up
     }

@@ -61,16 +61,30 @@ struct Stream<RNG_XORWOW> {
     }
 };
 
-// ---- Philox4x32-10: key = global stream id ^ seed; position = draws_done (R-C2) ----
+// ---- the 32-bit LCG (eq.(1), :46): the whole word is the draw ----
 template <>
-struct Stream<RNG_PHILOX4X32_10> {
+struct Stream<RNG_LCG32> {
+    uint32_t x;
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s) { x = ((const uint32_t *)g.state)[s]; }
+    __device__ __forceinline__ uint32_t next()
+    {
+        const uint32_t r = x;      // u_n = x_n / m, PAPER.md:35 (output, then advance: R-A3)
+        x = kLcg32A * x + kLcg32C; // eq.(1), m = 2^32
+        return r;
+    }
+    __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint32_t *)g.state)[s] = x; }
+};
+
+// ---- Philox4x32-R: key = global stream id ^ seed; position = draws_done (R-C2) ----
+template <int R>
+struct StreamPhilox {
     uint32_t k0, k1;
     uint64_t j; // next draw index
     uint4 buf;
     __device__ __forceinline__ void refill()
     {
         const uint64_t b = j >> 2;
-        buf = philox4x32<10>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
+        buf = philox4x32<R>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
     }
     __device__ __forceinline__ void load(const Gen &g, uint64_t s)
     {
@@ -88,6 +102,12 @@ struct Stream<RNG_PHILOX4X32_10> {
         return p == 0u ? buf.x : p == 1u ? buf.y : p == 2u ? buf.z : buf.w;
     }
     __device__ __forceinline__ void store(const Gen &, uint64_t) {}
+};
+template <>
+struct Stream<RNG_PHILOX4X32_10> : StreamPhilox<10> {
+};
+template <>
+struct Stream<RNG_PHILOX4X32_7> : StreamPhilox<7> {
 };
 
 // ---- XORShift1024/Weyl, cooperative: lane = word index; whole warps only ----

@@ -9,7 +9,7 @@ from __future__ import annotations
 
 from dataclasses import dataclass
 
-LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W = range(5)
+LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32 = range(7)
 MASTER_SEED = 1                    # "seeded via splitmix64(master seed 1)" (config 1)
 LATTICE_SEED = 2                   # ising_init_random seed
 BETA_C = 0.44068679350977147       # ln(1+sqrt 2)/2 as a double (config 5)
@@ -54,6 +54,13 @@ C4_DRAW = FillCfg("C4_xs1024_2^24x4096_draw", XS1024W, 1 << 24, 4096)
 # supplementary 4 GiB fills for the stateful per-thread generators (SURVEY.md 8(d) C1 note)
 C1_BIG = FillCfg("C1big_lcg64_2^20x1024", LCG64, 1 << 20, 1024)
 C3_FILL = FillCfg("C3fill_xorwow_2^20x1024", XORWOW, 1 << 20, 1024)
+# SURVEY.md 8(f)-1, the cheap extra kinds of the paper's Table 2, C2's shape
+N1_PHILOX7 = FillCfg("N1_philox7_2^20x1024", PHILOX4X32_7, 1 << 20, 1024)
+N1_LCG32 = FillCfg("N1_lcg32_2^20x1024", LCG32, 1 << 20, 1024)
+N1_PHILOX7_DRAW = FillCfg("N1_philox7_2^22x256", PHILOX4X32_7, 1 << 22, 256)
+N1_PHILOX10_DRAW = FillCfg("N1_philox10_2^22x256", PHILOX4X32_10, 1 << 22, 256)
+N1_LCG32_DRAW = FillCfg("N1_lcg32_2^22x256", LCG32, 1 << 22, 256)
+N1_LCG64_DRAW = FillCfg("N1_lcg64_2^22x256", LCG64, 1 << 22, 256)
 
 # C5a: L=4, beta=0.3 vs exact enumeration; 8 streams (K = 1 site per stream per colour)
 C5A_PHILOX = IsingCfg("C5a_ising_L4_philox", PHILOX4X32_10, 4, 0.3, 8, 1000)

@@ -61,6 +61,8 @@ def test_state_bytes(L):
     assert pkg.rng_state_bytes(pkg.RNG_XORWOW, 1 << 22) == 24 << 22  # "192 bits" PAPER.md:266
     assert pkg.rng_state_bytes(pkg.RNG_PHILOX4X32_10, 1 << 20) == 0   # no stored state
     assert pkg.rng_state_bytes(pkg.RNG_XS1024W, 1 << 24) == 4 << 24   # "32 bits/thread" PAPER.md:268
+    assert pkg.rng_state_bytes(pkg.RNG_PHILOX4X32_7, 1 << 20) == 0
+    assert pkg.rng_state_bytes(pkg.RNG_LCG32, 1000) == 4000            # "32 bits" PAPER.md:262 (Table 2)
     assert pkg.rng_state_bytes(99, 5) == 0
 
 
