@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
 
-LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W = range(5)
+LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32 = range(7)
 
 
 def build(force: bool = False) -> str:
@@ -63,6 +63,8 @@ def lib():
         L.orc_destroy.argtypes = [vp]
         L.orc_draws_done.restype = u64
         L.orc_draws_done.argtypes = [vp]
+        L.orc_set_draws_done.restype = C.c_int
+        L.orc_set_draws_done.argtypes = [vp, u64]
         for name in ("orc_fill_u32", "orc_fill_f32", "orc_draw_reduce"):
             f = getattr(L, name)
             f.restype = None
@@ -156,6 +158,11 @@ class Rng:
     @property
     def draws_done(self) -> int:
         return int(lib().orc_draws_done(self._h))
+
+    @draws_done.setter
+    def draws_done(self, v: int):
+        if lib().orc_set_draws_done(self._h, v) != 0:
+            raise ValueError("only counter-based (Philox) streams can be repositioned")
 
     def fill_u32(self, n: int) -> np.ndarray:
         out = np.empty(self.n_streams * n, dtype=np.uint32)

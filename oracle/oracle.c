@@ -244,6 +244,16 @@ void orc_destroy(orc_rng *r)
 
 uint64_t orc_draws_done(const orc_rng *r) { return r->draws_done; }
 
+/* Reposition a COUNTER-BASED stream: Philox has no state but (key, counter) and the
+ * counter is the draw index (R-C2), so any position is reachable at once.
+ * Stateful kinds cannot be repositioned this way: -1. */
+int orc_set_draws_done(orc_rng *r, uint64_t draws_done)
+{
+    if (r->kind != ORC_PHILOX4X32_10 && r->kind != ORC_PHILOX4X32_7) return -1;
+    r->draws_done = draws_done;
+    return 0;
+}
+
 /* Philox stream mapping (BASELINE.json config 2, R-C2): key = stream id XOR
  * seed (64 bit, k0 = low word); counter = index of the 4-word block,
  * (lo32(b), hi32(b), 0, 0); draw j is word (j mod 4) of block floor(j/4). */

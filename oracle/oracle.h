@@ -75,6 +75,8 @@ typedef struct orc_rng orc_rng;
 orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local, uint64_t seed);
 void     orc_destroy(orc_rng *);
 uint64_t orc_draws_done(const orc_rng *);
+/* Philox kinds only (the counter IS the position); others: returns -1 */
+int      orc_set_draws_done(orc_rng *, uint64_t draws_done);
 
 /* out[s*n + j] = draw (draws_done + j) of local stream s; then draws_done += n */
 void orc_fill_u32(orc_rng *, uint32_t *out, uint64_t n);

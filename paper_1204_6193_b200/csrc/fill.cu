@@ -113,6 +113,62 @@ __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_
     }
 }
 
+// Full tile whose blocks all share the high counter word (every tile except one per 2^32
+// blocks of a row): the structure of the counter (lo32(b), hi32(b), 0, 0) (R-C2) removes two
+// of the 2R multiplies of each block.
+//  * round 1: the second S-box multiplies zero; the first one, M0 * lo32(b), is linear in b:
+//    the lane's blocks are b, b+32, ..., so p0(b + 32u) = p0(b) + u * (32 M0) as 64-bit
+//    integers (lo32 does not wrap inside the tile): one IMAD.WIDE per lane and group, then
+//    64-bit additions on the otherwise half-idle alu pipe.
+//  * round 2: its first S-box input is hi32(b) ^ k0 (round 1 left c0 = hi(M1*0) ^ c1 ^ k0),
+//    the same for every block of the tile: one product per lane and group (`q`).
+// Rounds 3..R are the generic round.  Same bits as philox4x32<R> (tests compare both paths
+// with the oracle, also across a 2^32-block boundary).
+template <bool F32, int U, int R>
+__device__ __forceinline__ void philox_group_fast(uint32_t *__restrict__ row, uint32_t blo, uint32_t bhi, uint32_t rb0,
+                                                  const uint32_t (&rk0)[R], const uint32_t (&rk1)[R])
+{
+    static_assert(R >= 2, "needs two rounds");
+    uint32_t c0[U], c1[U], c2[U], c3[U];
+    const uint64_t p00 = (uint64_t)kPhM0 * blo;                       // round 1, block u = 0
+    const uint64_t q = (uint64_t)kPhM0 * (bhi ^ rk0[0]);              // round 2, first S-box: tile-uniform input
+    constexpr uint64_t STEP = 32ull * kPhM0;
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const uint64_t p0 = p00 + (uint64_t)u * STEP;                 // = M0 * (blo + 32u)
+        // after round 1: (c0,c1,c2,c3) = (bhi ^ k0, 0, hi(p0) ^ k1, lo(p0))
+        const uint32_t a2 = (uint32_t)(p0 >> 32) ^ rk1[0];
+        const uint32_t a3 = (uint32_t)p0;
+        // round 2
+        const uint64_t p1 = (uint64_t)kPhM1 * a2;
+        c0[u] = (uint32_t)(p1 >> 32) ^ rk0[1];                        // ^ c1 (= 0)
+        c2[u] = (uint32_t)(q >> 32) ^ a3 ^ rk1[1];
+        c1[u] = (uint32_t)p1;
+        c3[u] = (uint32_t)q;
+    }
+#pragma unroll
+    for (int r = 2; r < R; r++) {
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const uint64_t p0 = (uint64_t)kPhM0 * c0[u];
+            const uint64_t p1 = (uint64_t)kPhM1 * c2[u];
+            const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1[u] ^ rk0[r];
+            const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3[u] ^ rk1[r];
+            c1[u] = (uint32_t)p1;
+            c3[u] = (uint32_t)p0;
+            c0[u] = n0;
+            c2[u] = n2;
+        }
+    }
+    uint4 *dst = reinterpret_cast<uint4 *>(row) + rb0;
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const uint4 v = make_uint4(out_word(c0[u], F32), out_word(c1[u], F32), out_word(c2[u], F32),
+                                   out_word(c3[u], F32));
+        __stcs(dst + 32 * u, v);
+    }
+}
+
 template <bool F32, int U, int T, int R>
 __global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restrict__ out, uint64_t first, uint64_t seed,
                                                               uint64_t b0, uint64_t n, uint32_t blocks_per_row,
@@ -137,7 +193,15 @@ __global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restr
         }
         uint32_t *row = out + s * n;
         const bool tile_full = (uint64_t)(c + 1u) * (T * 32u * U) <= (uint64_t)blocks_per_row; // warp-uniform
-        if (tile_full) {
+        // first and last block index of the tile (warp-uniform); equal high words <=> lo32 does not wrap
+        const uint64_t bt0 = b0 + (uint64_t)c * (T * 32u * U), bt1 = bt0 + (T * 32u * U - 1u);
+        if (tile_full && (uint32_t)(bt0 >> 32) == (uint32_t)(bt1 >> 32)) {
+#pragma unroll 1
+            for (int g = 0; g < T; g++) {
+                const uint32_t rb0 = (c * T + g) * (32u * U) + lane;
+                philox_group_fast<F32, U, R>(row, (uint32_t)b0 + rb0, (uint32_t)(bt0 >> 32), rb0, rk0, rk1);
+            }
+        } else if (tile_full) {
 #pragma unroll 1
             for (int g = 0; g < T; g++)
                 philox_group<F32, U, false, R>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);

@@ -461,3 +461,30 @@ def test_table1_lcg64_substreams_fail_like_in_the_paper():
     e, e_err, _, _ = _table1_run(pkg.RNG_LCG64_LEAPFROG, 1 << 16, sweeps=50000, nb=50)
     print(f"\nlcg64_leapfrog: e = {e:.7f} +- {e_err:.7f} (exact {-exact['e']:.7f}, {(e + exact['e']) / e_err:+.1f} sigma)")
     assert (e - (-exact["e"])) > 10 * e_err
+
+
+@pytest.mark.parametrize("kind", [pkg.RNG_PHILOX4X32_10, pkg.RNG_PHILOX4X32_7], ids=["philox10", "philox7"])
+@pytest.mark.parametrize("f32", [False, True], ids=["u32", "f32"])
+def test_philox_fill_across_the_2_32_block_boundary(kind, f32):
+    """the fill kernel's fast path assumes one high counter word per tile (round-1 product by
+    increments, uniform round-2 product); the tile that straddles block 2^32 must take the
+    generic path, the tiles before and after it the fast one -- all against the oracle"""
+    S, seed, n = 5, 42, 8192                      # 2048 blocks per row = 8 tiles of 256 blocks
+    start = 4 * ((1 << 32) - 1000)                # the boundary falls inside the 4th tile
+    g, o = pkg.Rng(kind, S, seed), oracle.Rng(kind, S, seed)
+    g.draws_done = start
+    o.draws_done = start
+    if f32:
+        out = torch.empty(S * n, dtype=torch.float32, device="cuda")
+        g.fill_f32(out, n)
+        exp = o.fill_f32(n).view(np.uint32)
+    else:
+        out = dev_u32(S * n)
+        g.fill_u32(out, n)
+        exp = o.fill_u32(n)
+    got = out.cpu().numpy().view(np.uint32)[:S * n]
+    assert np.array_equal(got, exp), np.flatnonzero(got != exp)[:8]
+    red = dev_u32(2 * S)
+    g.draw_reduce(red, 4001)                      # draw mode across the same region
+    assert np.array_equal(host(red, 2 * S), o.draw_reduce(4001))
+    g.close()

@@ -189,3 +189,22 @@ def test_philox_high_counter_word_is_used():
     K = 9
     o = oracle.philox4x32([5, 1, 0, 0], [K, 0])
     assert not np.array_equal(o, oracle.philox4x32([5, 0, 0, 0], [K, 0]))
+
+
+def test_philox_repositioned_stream_crosses_the_2_32_block_boundary():
+    # the counter is the draw index (R-C2): a stream set to draw 4*(2^32 - 3) must produce the blocks
+    # (2^32-3, 0), (2^32-2, 0), (2^32-1, 0), (0, 1), (1, 1) of the elementary function (Ref.[20] KAT-pinned)
+    S, seed, start = 3, 0xABCDEF, 4 * ((1 << 32) - 3)
+    for kind, R in ((oracle.PHILOX4X32_10, 10), (oracle.PHILOX4X32_7, 7)):
+        r = oracle.Rng(kind, S, seed)
+        r.draws_done = start + 2                      # unaligned on purpose
+        out = r.fill_u32(18).reshape(S, 18)
+        assert r.draws_done == start + 20
+        for s in range(S):
+            K = s ^ seed
+            for j in range(18):
+                b = (start + 2 + j) // 4
+                o = oracle.philox4x32([b & M32, b >> 32, 0, 0], [K & M32, K >> 32], R)
+                assert out[s, j] == o[(start + 2 + j) % 4]
+    with pytest.raises(ValueError):
+        oracle.Rng(oracle.XORWOW, 4, 1).draws_done = 8   # stateful streams cannot be repositioned
