@@ -213,6 +213,12 @@ class IsingJob(Job):
         self.rng = pkg.Rng(cfg.kind, n_local, cfg.seed, first=first, n_total=n_total)
         self.spins = torch.empty(cfg.L * cfg.L, dtype=torch.int8, device="cuda")
         pkg.ising_init_random(self.spins, cfg.L, cfg.lattice_seed + rank)
+        # a half-sweep launch loads and stores every stream's state once: with few updates per
+        # stream (the paper's k = 1 regime) that traffic, not the arithmetic, bounds the kernel
+        self.K = cfg.L * cfg.L // 2 // cfg.n_streams
+        self.state_bytes_per_update = 2.0 * STATE_BYTES[cfg.kind] / self.K
+        if self.state_bytes_per_update >= 4.0:
+            self.bound = "hbm"
 
     def units_per_step(self):
         return float(self.cfg.L * self.cfg.L * self.sweeps)
@@ -222,6 +228,9 @@ class IsingJob(Job):
 
     def alg_per_launch(self):
         k = self.cfg.L * self.cfg.L // 2  # updates per half-sweep launch
+        if self.bound == "hbm":
+            # state load + store per stream, plus the two bit planes read and one written (1 bit per site)
+            return 2.0 * STATE_BYTES[self.cfg.kind] * self.cfg.n_streams + 3.0 * k / 8.0
         return (ALG_INST_PER_ISING_UPDATE + ALG_INST_PER_DRAW[self.cfg.kind]) * k
 
     def close(self):

@@ -188,7 +188,58 @@ __global__ void __launch_bounds__(128) ising_ms_word_kernel(Gen g, uint32_t *__r
     mw.load(Cp, Np, L, wpr, y, j, colour);
     uint32_t n0 = 0u, n1 = 0u;
     const uint64_t s0 = (uint64_t)widx * (32 / K);
-    if (kind_is_philox(KIND)) {
+    if (kind_is_philox(KIND) && (uint32_t)(g.first + s0) <= 0xffffffffu - 32u / K) {
+        // The 32/K streams of this word are consecutive ids sharing the high key word, and every
+        // stream is at the same counter (all streams advance in lockstep), so with the counter
+        // (lo32(b), hi32(b), 0, 0) of R-C2:
+        //  * round 1: M0 * lo32(b) is the same for every thread (uniform datapath) and M1 * 0 = 0;
+        //  * round 2: its second S-box input, hi(M0 lo32(b)) ^ k1, is shared by all streams of the word,
+        //    its first one, hi32(b) ^ k0, by all blocks of a stream;
+        //  * key schedule: k1 + r W1 once per word; k0 + r W0 once per stream, pinned to the alu pipe (the
+        //    multiplies fill the fma pipe: measured 1087 flips/ns with these adds on the fma pipe).
+        // Same bits as philox4x32<R> (the `else` branch and the byte kernels; tests compare all of them).
+        constexpr int R = philox_rounds(KIND);
+        constexpr int NS = 32 / K, NBS = K / 4;
+        const uint64_t b0 = g.draws_done >> 2; // draws_done % 4 == 0
+        const uint64_t id0 = (g.first + s0) ^ g.seed;
+        const uint32_t lo_id = (uint32_t)(g.first + s0), lo_seed = (uint32_t)g.seed;
+        const uint32_t zero = g.k_zero;
+        uint32_t rk1[R];
+#pragma unroll
+        for (int r = 0; r < R; r++) rk1[r] = (uint32_t)(id0 >> 32) + (uint32_t)r * kPhW1;
+#pragma unroll
+        for (int a = 0; a < NS; a++) {
+            const uint32_t k0 = (lo_id + (uint32_t)a) ^ lo_seed;
+            uint32_t rk0[R];
+            rk0[0] = k0;
+#pragma unroll
+            for (int r = 1; r < R; r++) rk0[r] = add_on_alu_pipe(k0, (uint32_t)r * kPhW0, zero);
+#pragma unroll
+            for (int j = 0; j < NBS; j++) {
+                const uint64_t ctr = b0 + (uint64_t)j;           // uniform
+                const uint64_t pu = (uint64_t)kPhM0 * (uint32_t)ctr; // uniform: round 1, first S-box
+                uint32_t c0 = (uint32_t)(ctr >> 32) ^ rk0[0];    // round 1 output: hi(M1*0) ^ c1 ^ k0
+                uint32_t c1 = 0u;
+                uint32_t c2 = (uint32_t)(pu >> 32) ^ rk1[0];
+                uint32_t c3 = (uint32_t)pu;
+#pragma unroll
+                for (int r = 1; r < R; r++) {
+                    const uint64_t p0 = (uint64_t)kPhM0 * c0;
+                    const uint64_t p1 = (uint64_t)kPhM1 * c2;
+                    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk0[r];
+                    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk1[r];
+                    c1 = (uint32_t)p1;
+                    c3 = (uint32_t)p0;
+                    c0 = n0;
+                    c2 = n2;
+                }
+                ms_cmp_insert(c0, thr, n0, n1);
+                ms_cmp_insert(c1, thr, n0, n1);
+                ms_cmp_insert(c2, thr, n0, n1);
+                ms_cmp_insert(c3, thr, n0, n1);
+            }
+        }
+    } else if (kind_is_philox(KIND)) {
         const uint64_t b0 = g.draws_done >> 2; // draws_done % 4 == 0
 #pragma unroll
         for (int gi = 0; gi < 8; gi++) {
