@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
 
-LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32 = range(7)
+LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP = range(8)
 
 
 def build(force: bool = False) -> str:
@@ -55,6 +55,10 @@ def lib():
         L.orc_xorwow_next.argtypes = [vp]
         L.orc_xs1024_update.restype = None
         L.orc_xs1024_update.argtypes = [vp]
+        for f, a in (("orc_xs1024_matrix", [vp]), ("orc_xs1024_vecmat", [vp, vp, vp]),
+                     ("orc_xs1024_matmul", [vp, vp, vp]), ("orc_xs1024_matpow2", [C.c_uint, vp])):
+            getattr(L, f).restype = None
+            getattr(L, f).argtypes = a
         L.orc_u32_to_f32.restype = C.c_float
         L.orc_u32_to_f32.argtypes = [u32]
         L.orc_create.restype = vp
@@ -122,6 +126,25 @@ def xorwow_next(state: np.ndarray) -> int:
     """advances `state` (6 x uint32, in place) and returns the draw."""
     assert state.dtype == np.uint32 and state.size == 6
     return int(lib().orc_xorwow_next(_p(state)))
+
+
+def xs1024_matpow2(k: int) -> np.ndarray:
+    """M^(2^k) as a [1024, 32] uint32 bit matrix (row r = image of unit vector word r//32, bit r%32)"""
+    out = np.empty((1024, 32), dtype=np.uint32)
+    lib().orc_xs1024_matpow2(k, _p(out))
+    return out
+
+
+def xs1024_matmul(A: np.ndarray, B: np.ndarray) -> np.ndarray:
+    out = np.empty((1024, 32), dtype=np.uint32)
+    lib().orc_xs1024_matmul(_p(np.ascontiguousarray(A)), _p(np.ascontiguousarray(B)), _p(out))
+    return out
+
+
+def xs1024_vecmat(X: np.ndarray, A: np.ndarray) -> np.ndarray:
+    out = np.empty(32, dtype=np.uint32)
+    lib().orc_xs1024_vecmat(_p(np.ascontiguousarray(X, dtype=np.uint32)), _p(np.ascontiguousarray(A)), _p(out))
+    return out
 
 
 def xs1024_update(X: np.ndarray) -> None:

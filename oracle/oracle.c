@@ -153,6 +153,47 @@ void orc_xs1024_update(uint32_t X[32])
     shr1024(X, 347, T); for (int i = 0; i < 32; i++) X[i] ^= T[i];
     shl1024(X, 344, T); for (int i = 0; i < 32; i++) X[i] ^= T[i];
 }
+/* ---- skip-ahead of the XORShift1024 ---------------------------
+ * The update is X <- X M over GF(2) (eq.(8)).  The paper seeds the
+ * instances by "multiplying the state with the precomputed 2^137-th power of the
+ * recursion matrix M".  Written out: M as 1024 rows of 1024 bits, row r = image
+ * of the unit vector e_r (word r/32, bit r%32 of that word) under ONE update;
+ * a vector-matrix product X A = XOR of the rows A[r] over the set bits r of X;
+ * a matrix product (A B)[r] = A[r] B; powers by repeated squaring. */
+void orc_xs1024_matrix(uint32_t *M /* [1024][32] */)
+{
+    for (int r = 0; r < 1024; r++) {
+        uint32_t *row = M + 32 * r;
+        memset(row, 0, 32 * sizeof(uint32_t));
+        row[r / 32] = 1u << (r % 32);
+        orc_xs1024_update(row);
+    }
+}
+void orc_xs1024_vecmat(const uint32_t X[32], const uint32_t *A, uint32_t out[32])
+{
+    uint32_t acc[32] = {0};
+    for (int r = 0; r < 1024; r++)
+        if ((X[r / 32] >> (r % 32)) & 1u)
+            for (int i = 0; i < 32; i++) acc[i] ^= A[32 * r + i];
+    memcpy(out, acc, sizeof acc);
+}
+void orc_xs1024_matmul(const uint32_t *A, const uint32_t *B, uint32_t *out /* may not alias */)
+{
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < 1024; r++) orc_xs1024_vecmat(A + 32 * r, B, out + 32 * r);
+}
+/* out = M^(2^k) by k squarings */
+void orc_xs1024_matpow2(unsigned k, uint32_t *out /* [1024][32] */)
+{
+    uint32_t *T = (uint32_t *)malloc(1024 * 32 * sizeof(uint32_t));
+    orc_xs1024_matrix(out);
+    for (unsigned i = 0; i < k; i++) {
+        orc_xs1024_matmul(out, out, T);
+        memcpy(out, T, 1024 * 32 * sizeof(uint32_t));
+    }
+    free(T);
+}
+
 /* Weyl part, eq.(9): y_n = y_0 + n c mod 2^32, c = 362437;
  * R-D6: y_0 = 0 for every instance (footnote 4), n = number of
  * updates since creation.  Output (gamma = w/2 = 16):
@@ -186,8 +227,8 @@ uint32_t orc_lcg32_step(uint32_t x) { return 1664525u * x + 1013904223u; }
 orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local, uint64_t seed)
 {
     if (n_local < 1 || first + n_local > n_total || first + n_local < first) return NULL;
-    if (kind < ORC_LCG64 || kind > ORC_LCG32) return NULL;
-    if (kind == ORC_XS1024W && (first % 32 || n_local % 32)) return NULL;
+    if (kind < ORC_LCG64 || kind > ORC_XS1024W_SKIP) return NULL;
+    if ((kind == ORC_XS1024W || kind == ORC_XS1024W_SKIP) && (first % 32 || n_local % 32)) return NULL;
     orc_rng *r = (orc_rng *)calloc(1, sizeof *r);
     if (!r) return NULL;
     r->kind = kind; r->n_total = n_total; r->first = first; r->n_local = n_local; r->seed = seed;
@@ -232,6 +273,29 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
             if (!any) X[31] = 1;
         }
         break;
+    case ORC_XS1024W_SKIP: {
+        /* every instance starts from the SAME state and skips g * 2^137 updates,
+         * g = global instance number, by multiplying with J = M^(2^137) once per instance.
+         * R-D7b: the paper does not say which common state; it is instance 0's state under
+         * the random seeding above (SM_seed[0..15]). */
+        uint32_t *J = (uint32_t *)malloc(1024 * 32 * sizeof(uint32_t));
+        uint32_t X[32], any = 0;
+        orc_xs1024_matpow2(137, J);
+        for (int k = 0; k < 16; k++) {
+            uint64_t z = orc_splitmix64(seed, (uint64_t)k);
+            X[2 * k] = (uint32_t)z;
+            X[2 * k + 1] = (uint32_t)(z >> 32);
+            any |= X[2 * k] | X[2 * k + 1];
+        }
+        if (!any) X[31] = 1;
+        r->xs = (uint32_t *)malloc(n_local * sizeof(uint32_t));
+        for (uint64_t gg = 0; gg < (first + n_local) / 32; gg++) { /* successively, as the paper does */
+            if (gg >= first / 32) memcpy(r->xs + 32 * (gg - first / 32), X, sizeof X);
+            orc_xs1024_vecmat(X, J, X);
+        }
+        free(J);
+        break;
+    }
     }
     return r;
 }
@@ -322,6 +386,7 @@ void orc_fill_u32(orc_rng *r, uint32_t *out, uint64_t n)
         }
         break;
     case ORC_XS1024W:
+    case ORC_XS1024W_SKIP:
         /* stream s = word (s mod 32) of instance floor(s/32)  (R-D4) */
 #pragma omp parallel for schedule(static)
         for (uint64_t g = 0; g < S / 32; g++) {
@@ -373,7 +438,7 @@ uint64_t orc_state_words32(const orc_rng *r)
     switch (r->kind) {
     case ORC_LCG64: case ORC_LCG64_LEAPFROG: return 2 * r->n_local;
     case ORC_XORWOW: return 6 * r->n_local;
-    case ORC_XS1024W: return r->n_local;
+    case ORC_XS1024W: case ORC_XS1024W_SKIP: return r->n_local;
     case ORC_LCG32: return r->n_local;
     default: return 0;
     }
@@ -392,7 +457,7 @@ void orc_get_state(const orc_rng *r, uint32_t *out)
         break;
     }
     case ORC_XORWOW: memcpy(out, r->xw, r->n_local * 24); break;
-    case ORC_XS1024W: memcpy(out, r->xs, r->n_local * 4); break;
+    case ORC_XS1024W: case ORC_XS1024W_SKIP: memcpy(out, r->xs, r->n_local * 4); break;
     case ORC_LCG32: memcpy(out, r->lcg32, r->n_local * 4); break;
     default: break;
     }

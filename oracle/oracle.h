@@ -34,8 +34,10 @@ enum {
     ORC_PHILOX4X32_10  = 3, /* PAPER.md:284-296 (constants: Ref.[20], R-C1)     */
     ORC_XS1024W        = 4, /* PAPER.md:166 eq.(8), :177, :201-225, :232-240    */
     ORC_PHILOX4X32_7   = 5, /* the 7-round variant          */
-    ORC_LCG32          = 6  /* PAPER.md:33 eq.(1), :46: a=1664525, c=1013904223,
+    ORC_LCG32          = 6, /* PAPER.md:33 eq.(1), :46: a=1664525, c=1013904223,
                                m=2^32; draw j = x_j (all 32 bits), x_0 = lo32(SM_seed[s]) */
+    ORC_XS1024W_SKIP   = 7  /* kind 4 seeded as PAPER.md:228 does: all instances from one
+                               state, instance g skipped ahead by g * 2^137 updates     */
 };
 
 /* ---- elementary pieces, exported so that the tests can pin them ---------- */
@@ -61,6 +63,14 @@ uint32_t orc_xorwow_next(uint32_t st[6]);
 /* one update X <- X M of the 1024-bit XORShift, eq.(8) with (a,b,c) =
  * (329,347,344); X[0] is the MOST significant word (R-D1). */
 void orc_xs1024_update(uint32_t X[32]);
+
+/* skip-ahead: M as a bit matrix (row r = image of the unit vector
+ * "word r/32, bit r%32" under one update), X A, A B, and M^(2^k) by k squarings.
+ * Matrices are [1024][32] uint32, row-major. */
+void orc_xs1024_matrix(uint32_t *M);
+void orc_xs1024_vecmat(const uint32_t X[32], const uint32_t *A, uint32_t out[32]);
+void orc_xs1024_matmul(const uint32_t *A, const uint32_t *B, uint32_t *out);
+void orc_xs1024_matpow2(unsigned k, uint32_t *out);
 
 /* fixed output map u32 -> [0,1) float:  (u >> 8) * 2^-24   (BASELINE.json) */
 float orc_u32_to_f32(uint32_t u);
