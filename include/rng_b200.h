@@ -85,7 +85,15 @@ enum {
      * (Table 2 "LCG32"): draw j = x_j, the whole word (u = x/m, PAPER.md:35;
      * output, then advance); x_0 of stream s = lo32(SM_seed[s]).  Period 2^32: the paper's
      * deliberately bad example (fails SmallCrush), here for its Table-2 row. */
-    RNG_LCG32 = 6
+    RNG_LCG32 = 6,
+    /* kind 4's generator seeded the way the paper itself seeds it: every
+     * instance starts from ONE common state X_0 and instance g (global number, streams
+     * 32g..32g+31) skips g * 2^137 updates: X_g = X_0 M^(g 2^137), M the 1024x1024 GF(2) matrix
+     * of one update.  The sub-streams of 2^137 numbers are consecutive blocks of one sequence
+     * and cannot overlap.  X_0 = kind 4's instance 0 (SM_seed[0..15], R-D7b).  Update, Weyl
+     * term (the same for all instances: footnote 4), output, layout, state
+     * access and every entry point are exactly kind 4's. */
+    RNG_XS1024W_SKIP = 7
 };
 
 enum {

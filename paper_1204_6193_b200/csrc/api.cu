@@ -71,6 +71,7 @@ uint64_t rng_state_bytes(int kind, uint64_t n)
     case RNG_LCG64_LEAPFROG: return 8 * n;
     case RNG_XORWOW: return 24 * n;
     case RNG_XS1024W:
+    case RNG_XS1024W_SKIP:
     case RNG_LCG32: return 4 * n;
     default: return 0;
     }
@@ -80,11 +81,11 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
 {
     if (!out) return fail(RNG_E_INVAL, "rng_create: out is NULL");
     *out = nullptr;
-    if (kind < RNG_LCG64 || kind > RNG_LCG32) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
+    if (kind < RNG_LCG64 || kind > RNG_XS1024W_SKIP) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
     if (n_local < 1 || first + n_local < first || first + n_local > n_total)
         return fail(RNG_E_INVAL, "rng_create: stream range [%llu,+%llu) not inside [0,%llu)", (unsigned long long)first,
                     (unsigned long long)n_local, (unsigned long long)n_total);
-    if (kind == RNG_XS1024W && ((first | n_local) & 31ull))
+    if ((kind == RNG_XS1024W || kind == RNG_XS1024W_SKIP) && ((first | n_local) & 31ull))
         return fail(RNG_E_INVAL, "rng_create: RNG_XS1024W needs whole 32-stream instances");
     if (n_local > (1ull << 38)) return fail(RNG_E_INVAL, "rng_create: too many streams");
     int dev = 0, ndev = 0;
@@ -97,7 +98,8 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
     if (!h) return fail(RNG_E_NOMEM, "rng_create: host allocation failed");
     memset(h, 0, sizeof *h);
     h->device = dev;
-    h->g.kind = kind;
+    h->api_kind = kind;
+    h->g.kind = (kind == RNG_XS1024W_SKIP) ? RNG_XS1024W : kind; // same generator, other seeding
     h->g.S = n_local;
     h->g.first = first;
     h->g.n_total = n_total;
@@ -112,7 +114,7 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
     if (e == cudaSuccess && (kind == RNG_LCG64 || kind == RNG_LCG64_LEAPFROG)) e = cudaMalloc(&tab, sizeof(LcgTable));
     h->g.lcg = tab;
     if (e == cudaSuccess) e = cudaMalloc(&h->energy_scratch, sizeof(int64_t));
-    if (e == cudaSuccess) e = launch_seed(h->g, tab, 0);
+    if (e == cudaSuccess) e = (kind == RNG_XS1024W_SKIP) ? launch_seed_xs1024_skip(h->g, 0) : launch_seed(h->g, tab, 0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(0);
     if (e != cudaSuccess) {
         int rc = cuda_fail(e, "rng_create");

@@ -50,6 +50,7 @@ struct rng_handle {
     uint32_t *ms_planes;     // device scratch of the multi-spin Ising path: two bit planes of L*L/64 words
     uint64_t ms_planes_bytes;
     int var_xs1024, var_ising, var_store, var_lcg;
+    int api_kind; // the kind rng_create was called with (g.kind is RNG_XS1024W for RNG_XS1024W_SKIP)
 };
 
 // run MACRO(KIND) for the runtime kind (every kind that has a Stream<KIND>)
@@ -71,6 +72,8 @@ void count_launch(uint64_t n = 1);
 
 // seed.cu
 cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st);
+// seed_xs1024_skip.cu (RNG_XS1024W_SKIP; synchronises the stream, frees its scratch)
+cudaError_t launch_seed_xs1024_skip(const Gen &g, cudaStream_t st);
 // fill.cu  (f32 = apply the (u>>8)*2^-24 map; out is uint32_t* or float*)
 cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st);
 // fill_xs1024.cu (XORShift1024/Weyl, K words per lane; variant "xs1024" = K, 64 = the generic kernels)

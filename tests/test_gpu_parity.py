@@ -14,6 +14,7 @@ import paper_1204_6193_b200 as pkg  # noqa: E402
 
 KINDS = list(pkg.KIND_NAMES)
 IDS = [pkg.KIND_NAMES[k] for k in KINDS]
+XS_KINDS = (pkg.RNG_XS1024W, pkg.RNG_XS1024W_SKIP)
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -36,7 +37,7 @@ def host(t, n, dtype=np.uint32):
 
 
 def n_streams_for(kind, S):
-    return S - S % 32 if kind == pkg.RNG_XS1024W else S
+    return S - S % 32 if kind in XS_KINDS else S
 
 
 # ---------------------------------------------------------------------------------
@@ -264,7 +265,7 @@ def test_ising_init_and_energy():
                                         (128, 32, 4), (256, 4096, 5), (512, 16384, 3), (48, 96, 5), (64, 512, 4),
                                         (1024, 1024, 2)])
 def test_ising_sweep_bit_exact(kind, L, S, sweeps):
-    if kind == pkg.RNG_XS1024W and S % 32:
+    if kind in XS_KINDS and S % 32:
         pytest.skip("xs1024 needs whole 32-stream instances")
     beta = 0.3 if L == 4 else 0.44068679350977147
     g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
@@ -293,7 +294,7 @@ def test_ising_sweep_bit_exact(kind, L, S, sweeps):
 def test_ising_kernel_variants_share_one_trajectory(kind, L, S, sweeps, variant):
     """every kernel variant (generic byte kernel, 16-byte chunk kernel, multi-spin bit planes in
     STREAM and WORD mode) reproduces the oracle's lattice, energy trace and generator state"""
-    if kind == pkg.RNG_XS1024W and S % 32:
+    if kind in XS_KINDS and S % 32:
         pytest.skip("xs1024 needs whole 32-stream instances")
     beta = 0.44068679350977147
     g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
@@ -488,3 +489,27 @@ def test_philox_fill_across_the_2_32_block_boundary(kind, f32):
     g.draw_reduce(red, 4001)                      # draw mode across the same region
     assert np.array_equal(host(red, 2 * S), o.draw_reduce(4001))
     g.close()
+
+
+def test_xs1024_skip_seeding_large_shard_against_the_skip_matrix():
+    """PAPER.md:228 at a size where the doubling tree has many levels and a ragged last one, for a
+    shard whose first instance has several set bits: sampled instances against X_0 J^g computed with
+    the oracle's matrix powers (J^g by binary exponentiation over the oracle's J_k = M^(2^(137+k)))"""
+    n_inst, G0, seed = 3000, 0b1011010, 5
+    g = pkg.Rng(pkg.RNG_XS1024W_SKIP, 32 * n_inst, seed, first=32 * G0, n_total=32 * (G0 + n_inst))
+    st = g.get_state().reshape(n_inst, 32)
+    g.close()
+    x0 = oracle.Rng(oracle.XS1024W, 32, seed).get_state()
+    Jk = [oracle.xs1024_matpow2(137)]
+    for _ in range(12):
+        Jk.append(oracle.xs1024_matmul(Jk[-1], Jk[-1]))
+
+    def inst(G):
+        X = x0
+        for k in range(13):
+            if (G >> k) & 1:
+                X = oracle.xs1024_vecmat(X, Jk[k])
+        return X
+    for i in (0, 1, 2, 3, 63, 64, 1023, 1024, 2047, 2048, 2999):
+        assert np.array_equal(st[i], inst(G0 + i)), i
+    assert len({st[i].tobytes() for i in range(n_inst)}) == n_inst
