@@ -2,6 +2,8 @@
 // that never leave the register file and reduces them to {XOR, SUM mod 2^32}.  This is the
 // regime of the paper's peak numbers ("compute-bound"): the only memory
 // traffic is one state load and one state store per stream plus 8 bytes out.
+#include <type_traits>
+
 #include "internal.h"
 #include "streams.cuh"
 
@@ -68,11 +70,65 @@ __global__ void __launch_bounds__(256) philox_draw_reduce_kernel(Gen g, uint2 *_
             sum += w[j & 3ull];
         }
     }
-    for (; j + 4 <= end; j += 4) {
-        const uint64_t b = j >> 2;
-        const uint4 r = philox4x32<R>((uint32_t)b, (uint32_t)(b >> 32), 0u, 0u, k0, k1);
-        x ^= r.x ^ r.y ^ r.z ^ r.w;
-        sum += r.x + r.y + r.z + r.w;
+    // whole blocks.  The counter is (lo32(b), hi32(b), 0, 0) (R-C2) and b advances by one: round 1's
+    // only non-zero product M0 * lo32(b) grows by M0 per block (a 64-bit add instead of a multiply) and
+    // round 2's first product M0 * (hi32(b) ^ k0) is constant while hi32(b) is (see philox_group_fast in
+    // fill.cu); both are re-derived whenever lo32(b) wraps.  2R - 2 multiplies per block instead of 2R.
+    if (j + 4 <= end) {
+        uint64_t b = j >> 2;
+        const uint64_t b_end = end >> 2; // first block that is not whole
+        uint32_t rk0[R], rk1[R];
+#pragma unroll
+        for (int r = 0; r < R; r++) rk0[r] = k0 + (uint32_t)r * kPhW0, rk1[r] = k1 + (uint32_t)r * kPhW1;
+        while (b < b_end) {
+            const uint32_t bhi = (uint32_t)(b >> 32);
+            uint64_t seg = (((uint64_t)bhi + 1ull) << 32) - b; // blocks left with this high word
+            if (seg > b_end - b) seg = b_end - b;
+            uint64_t p0 = (uint64_t)kPhM0 * (uint32_t)b;
+            const uint64_t q = (uint64_t)kPhM0 * (bhi ^ rk0[0]);
+            b += seg;
+            // U blocks interleaved per trip: the ten rounds of one block are a dependent chain
+            constexpr int U = 2;
+            auto blocks = [&](auto nblk) {
+                constexpr int NB = decltype(nblk)::value;
+                uint32_t c0[NB], c1[NB], c2[NB], c3[NB];
+#pragma unroll
+                for (int u = 0; u < NB; u++) {
+                    const uint64_t pu = p0 + (uint64_t)u * (uint64_t)kPhM0; // = M0 * lo32(b + u)
+                    // after round 1: (c0,c1,c2,c3) = (bhi ^ k0, 0, hi(pu) ^ k1, lo(pu)); round 2:
+                    const uint32_t a2 = (uint32_t)(pu >> 32) ^ rk1[0];
+                    const uint64_t p1 = (uint64_t)kPhM1 * a2;
+                    c0[u] = (uint32_t)(p1 >> 32) ^ rk0[1];
+                    c2[u] = (uint32_t)(q >> 32) ^ (uint32_t)pu ^ rk1[1];
+                    c1[u] = (uint32_t)p1, c3[u] = (uint32_t)q;
+                }
+#pragma unroll
+                for (int r = 2; r < R; r++) {
+#pragma unroll
+                    for (int u = 0; u < NB; u++) {
+                        const uint64_t m0 = (uint64_t)kPhM0 * c0[u];
+                        const uint64_t m1 = (uint64_t)kPhM1 * c2[u];
+                        const uint32_t n0 = (uint32_t)(m1 >> 32) ^ c1[u] ^ rk0[r];
+                        const uint32_t n2 = (uint32_t)(m0 >> 32) ^ c3[u] ^ rk1[r];
+                        c1[u] = (uint32_t)m1, c3[u] = (uint32_t)m0, c0[u] = n0, c2[u] = n2;
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < NB; u++) {
+                    x ^= c0[u] ^ c1[u] ^ c2[u] ^ c3[u];
+                    sum += c0[u] + c1[u] + c2[u] + c3[u];
+                }
+                p0 += (uint64_t)NB * (uint64_t)kPhM0;
+            };
+            while (seg) { // 32-bit trip counts
+                const uint32_t s32 = seg > 0x40000000ull ? 0x40000000u : (uint32_t)seg;
+                seg -= s32;
+#pragma unroll 1
+                for (uint32_t t = 0; t < s32 / U; t++) blocks(std::integral_constant<int, U>{});
+                if (s32 % U) blocks(std::integral_constant<int, 1>{});
+            }
+        }
+        j = b_end << 2;
     }
     if (j < end) { // tail
         const uint64_t b = j >> 2;

@@ -486,8 +486,11 @@ def test_philox_fill_across_the_2_32_block_boundary(kind, f32):
     got = out.cpu().numpy().view(np.uint32)[:S * n]
     assert np.array_equal(got, exp), np.flatnonzero(got != exp)[:8]
     red = dev_u32(2 * S)
-    g.draw_reduce(red, 4001)                      # draw mode across the same region
-    assert np.array_equal(host(red, 2 * S), o.draw_reduce(4001))
+    for pos in (4 * ((1 << 32) - 500) + 1, 4 * ((1 << 32) - 1), 4 * (1 << 32), 4 * ((1 << 33) - 700) + 3):
+        g.draws_done = pos                        # draw mode: unaligned head, the wrap inside, ragged tail
+        o.draws_done = pos
+        g.draw_reduce(red, 4001)
+        assert np.array_equal(host(red, 2 * S), o.draw_reduce(4001)), pos
     g.close()
 
 
