@@ -197,6 +197,36 @@ class DrawJob(Job):
         self.rng.close()
 
 
+class SeedJob(Job):
+    """row a1: one step = rng_create (allocate + seed every stream; synchronous) + rng_destroy.
+    Unit: streams seeded per second.  Bound by launch count and allocation for the random
+    seeding, by the vector-matrix products for the paper's skip-ahead."""
+    bound = "alu"
+    unit = "Gstreams/s"
+    dtype = "u32"
+
+    def __init__(self, name: str, kind: int, n_streams: int, rank: int, world: int):
+        from paper_1204_6193_b200.sharding import weak_scaling_shard
+        self.name, self.kind = name, kind
+        self.n_total, self.first, self.n_local = weak_scaling_shard(rank, world, n_streams)
+
+    def units_per_step(self):
+        return float(self.n_local)
+
+    def step(self):
+        import paper_1204_6193_b200 as pkg
+        pkg.Rng(self.kind, self.n_local, W.MASTER_SEED, first=self.first, n_total=self.n_total).close()
+
+    def alg_per_launch(self):
+        # skip-ahead: one vector-matrix product per instance = 1024 predicated loads + 512 xors (average) per
+        # 32 streams; random seeding: 16 splitmix64 outputs of ~10 instructions per instance
+        per_inst = 1536.0 * 32 if self.kind == W.XS1024W_SKIP else 160.0
+        return per_inst * self.n_local / 32.0
+
+    def close(self):
+        pass
+
+
 class IsingJob(Job):
     bound = "alu"
     unit = "flips/ns"
@@ -274,7 +304,7 @@ def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, 
            "ms_per_step": ms / steps, "gpu_launches": int(launches), "dtype": job.dtype}
     # roofline of the (single) dominant kernel: average launch duration = timed region / launches
     peaks = measured_peaks()
-    n_l = max(int(launches), 1)
+    n_l = steps if isinstance(job, SeedJob) else max(int(launches), 1)  # SeedJob counts per step (many small launches)
     sec_per_launch = ms * 1e-3 / n_l
     if job.bound == "hbm":
         ach = job.alg_per_launch() / sec_per_launch / 1e9
@@ -312,6 +342,8 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
         "C3_draw": lambda: DrawJob(W.C3, rank, world, buf),
         "C4_fill": lambda: FillJob(W.C4_FILL, False, rank, world, buf),
         "C4_draw": lambda: DrawJob(W.C4_DRAW, rank, world, buf),
+        "N2_seed_xs1024_random": lambda: SeedJob("N2_seed_xs1024_random_2^24", W.XS1024W, 1 << 24, rank, world),
+        "N2_seed_xs1024_skip": lambda: SeedJob("N2_seed_xs1024_skip_2^24", W.XS1024W_SKIP, 1 << 24, rank, world),
         "C5b_philox": lambda: IsingJob(W.C5B_PHILOX, rank, world, ising_sweeps),
         "C5b_xorwow": lambda: IsingJob(W.C5B_XORWOW, rank, world, ising_sweeps),
         "C5b_xorwow_K8": lambda: IsingJob(W.C5B_XORWOW_K8, rank, world, ising_sweeps),
@@ -327,7 +359,8 @@ SUITE = [("C2_f32", 20, 3), ("C1_u32", 200, 10), ("C1_f32", 200, 10), ("C1big_u3
          ("C3_draw", 20, 3), ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1),
          ("C5b_xorwow_K8", 1, 1),
          ("N1_philox7_u32", 20, 3), ("N1_lcg32_u32", 20, 3), ("N1_philox7_draw", 20, 3), ("N1_philox10_draw", 20, 3),
-         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3)]
+         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3),
+         ("N2_seed_xs1024_random", 5, 3), ("N2_seed_xs1024_skip", 5, 3)]
 
 
 # ------------------------------------------------------------------------------------

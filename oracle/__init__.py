@@ -85,6 +85,8 @@ def lib():
         L.orc_ising_energy.argtypes = [vp, u32]
         L.orc_ising_sweep.restype = i32
         L.orc_ising_sweep.argtypes = [vp, vp, u32, C.c_double, u32, vp]
+        L.orc_ising_sweep_multihit.restype = i32
+        L.orc_ising_sweep_multihit.argtypes = [vp, vp, u32, C.c_double, u32, u32, u32, vp]
         L.orc_threads.restype = i32
         L.orc_set_threads.argtypes = [i32]
         _lib = L
@@ -213,6 +215,16 @@ class Rng:
         rc = lib().orc_ising_sweep(self._h, _p(spins), L, float(beta), n_sweeps, _p(tr) if trace else None)
         if rc != 0:
             raise ValueError("orc_ising_sweep: invalid arguments")
+        return tr
+
+    def ising_sweep_multihit(self, spins: np.ndarray, L: int, beta: float, n_sweeps: int, tile: int, k_hits: int,
+                             trace: bool = False):
+        assert spins.dtype == np.int8 and spins.size == L * L and spins.flags.c_contiguous
+        tr = np.empty(n_sweeps, dtype=np.int64) if trace else None
+        rc = lib().orc_ising_sweep_multihit(self._h, _p(spins), L, float(beta), n_sweeps, tile, k_hits,
+                                            _p(tr) if trace else None)
+        if rc != 0:
+            raise ValueError("orc_ising_sweep_multihit: invalid arguments")
         return tr
 
 

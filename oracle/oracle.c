@@ -548,3 +548,58 @@ void orc_set_threads(int n)
     (void)n;
 #endif
 }
+
+/* ---- the paper's own consumer: double checkerboard with multi-hit updates --------
+ * PAPER.md:56 ("a double checkerboard decomposition"), :58 ("updating the spins of a
+ * tile once (k = 1) ... two random numbers are produced per state load ... multi-hit
+ * updates (k = 100), 200 random numbers"); the kernel itself is in Refs.[13,25], so the
+ * order below is reading R-E9:
+ *   the lattice is cut into T x T tiles (T even, L/T even); tile (tx,ty) has COARSE colour
+ *   (tx+ty)&1.  One sweep = coarse colour 0, then coarse colour 1.  For one coarse colour,
+ *   every tile of that colour (they are independent: all sites around a tile belong to
+ *   tiles of the other coarse colour, which rest) receives k HITS; a hit = update all sites
+ *   of fine colour 0 of the tile, then all of fine colour 1 (fine colour = (x+y)&1, the
+ *   usual checkerboard), each by the Metropolis rule of orc_ising_sweep.
+ * Streams (one per thread of the paper's kernel: 1024^2 sites <-> 262144 threads,
+ * PAPER.md:54): S = L*L/4.  Tiles of one coarse colour are numbered p = ty*(L/T/2) + txh,
+ * tx = 2*txh + ((ty+C)&1); thread t < T*T/2 of a tile owns the fine-colour-c site
+ * y_l = t/(T/2), x_l = 2*(t%(T/2)) + ((y_l+c)&1) for c = 0 and 1 (a horizontal domino);
+ * stream s = p*(T*T/2) + t serves tile p of BOTH coarse colours.  Per sweep a stream
+ * spends 4k draws in the order (C, hit, c): draw ((2*sweep + C)*k + hit)*2 + c.  */
+int orc_ising_sweep_multihit(orc_rng *r, int8_t *sp, uint32_t L, double beta, uint32_t n_sweeps,
+                             uint32_t T, uint32_t k_hits, int64_t *trace)
+{
+    if (!r || T < 2 || (T & 1) || L % T || ((L / T) & 1) || k_hits < 1) return -1;
+    const uint64_t S = r->n_local, tpt = (uint64_t)T * T / 2; /* threads per tile */
+    if (S != (uint64_t)L * L / 4) return -1;
+    const uint32_t ntx = L / T, nth = ntx / 2;
+    float P[5];
+    orc_ising_accept_table(beta, P);
+    uint32_t *draws = (uint32_t *)malloc(S * 2 * sizeof(uint32_t));
+    if (!draws) return -1;
+    for (uint32_t sw = 0; sw < n_sweeps; sw++) {
+        for (uint32_t C = 0; C < 2; C++)
+            for (uint32_t hit = 0; hit < k_hits; hit++) {
+                orc_fill_u32(r, draws, 2); /* draws[2 s + c]: the stream's next two numbers */
+                for (uint32_t c = 0; c < 2; c++) {
+#pragma omp parallel for schedule(static)
+                    for (uint64_t s = 0; s < S; s++) {
+                        uint64_t p = s / tpt, t = s % tpt;
+                        uint32_t ty = (uint32_t)(p / nth), txh = (uint32_t)(p % nth);
+                        uint32_t tx = 2 * txh + ((ty + C) & 1);
+                        uint32_t yl = (uint32_t)(t / (T / 2)), xl = 2 * (uint32_t)(t % (T / 2)) + ((yl + c) & 1);
+                        uint64_t x = (uint64_t)tx * T + xl, y = (uint64_t)ty * T + yl;
+                        int sc = sp[y * L + x];
+                        int nn = sp[y * L + (x + 1) % L] + sp[y * L + (x + L - 1) % L]
+                               + sp[((y + 1) % L) * L + x] + sp[((y + L - 1) % L) * L + x];
+                        int h = sc * nn;
+                        float u = orc_u32_to_f32(draws[2 * s + c]);
+                        if (u < P[(h + 4) / 2]) sp[y * L + x] = (int8_t)(-sc);
+                    }
+                }
+            }
+        if (trace) trace[sw] = orc_ising_energy(sp, L);
+    }
+    free(draws);
+    return 0;
+}

@@ -117,6 +117,13 @@ int64_t orc_ising_energy(const int8_t *spins, uint32_t L);
 int orc_ising_sweep(orc_rng *, int8_t *spins, uint32_t L, double beta,
                     uint32_t n_sweeps, int64_t *energy_trace);
 
+/* The paper's own consumer (R-E9): double checkerboard of T x T tiles
+ * with k_hits multi-hit updates per tile visit; n_local must be L*L/4 (one stream per
+ * thread of the paper's kernel); T even, T | L, L/T even.  A sweep updates every site
+ * k_hits times and spends 4*k_hits draws per stream.  returns 0, or -1 on bad arguments. */
+int orc_ising_sweep_multihit(orc_rng *, int8_t *spins, uint32_t L, double beta, uint32_t n_sweeps,
+                             uint32_t T, uint32_t k_hits, int64_t *energy_trace);
+
 /* number of OpenMP threads the loops above will use (1 if built without) */
 int orc_threads(void);
 void orc_set_threads(int n);
