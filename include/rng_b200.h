@@ -151,6 +151,22 @@ int rng_draw_reduce(rng_handle *h, uint32_t *d_out, uint64_t n, void *cuda_strea
 int ising_sweep(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_t n_sweeps,
                 int64_t *d_energy_trace, void *cuda_stream);
 
+/* ---- a8': the paper's own consumer: double checkerboard with multi-hit updates -------
+ * (Table 1's k = 1 and k = 100 columns; reading R-E9.)
+ * The lattice is cut into tile x tile tiles (tile even, 2..44, tile | L, L/tile even);
+ * tile (tx,ty) has coarse colour (tx+ty)&1.  A sweep = coarse colour 0, then 1.  For one
+ * coarse colour every tile of that colour receives k_hits hits; a hit = all its sites of fine
+ * colour 0 ((x+y)&1 == 0), then all of fine colour 1, Metropolis rule and table as ising_sweep.
+ * Streams: n_local must equal L*L/4.  Tiles of one coarse colour are numbered
+ * p = ty*(L/tile/2) + txh, tx = 2*txh + ((ty+C)&1); thread t < tile*tile/2 owns, for c = 0, 1,
+ * the site y_l = t/(tile/2), x_l = 2*(t%(tile/2)) + ((y_l+c)&1) of the tile; stream
+ * s = p*tile*tile/2 + t serves tile p of both coarse colours and spends its draws in the order
+ * (coarse colour, hit, fine colour): 4*k_hits per sweep, 2*k_hits per generator state load.
+ * RNG_XS1024W / _SKIP need tile % 8 == 0.  d_energy_trace as in ising_sweep.
+ * draws_done += 4*k_hits*n_sweeps.  Errors: RNG_E_INVAL (geometry, stream count), RNG_E_CUDA. */
+int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_t n_sweeps,
+                         uint32_t tile, uint32_t k_hits, int64_t *d_energy_trace, void *cuda_stream);
+
 /* helpers (not hot path) */
 /* spin i = +1 if bit (i & 63) of SM_seed[i >> 6] is set, else -1 */
 int ising_init_random(int8_t *d_spins, uint32_t L, uint64_t seed, void *cuda_stream);

@@ -31,6 +31,7 @@ EXPORTS = {
     "rng_fill_f32": (_i32, [_vp, _vp, _u64, _vp]),
     "rng_draw_reduce": (_i32, [_vp, _vp, _u64, _vp]),
     "ising_sweep": (_i32, [_vp, _vp, _u32, _dbl, _u32, _vp, _vp]),
+    "ising_sweep_multihit": (_i32, [_vp, _vp, _u32, _dbl, _u32, _u32, _u32, _vp, _vp]),
     "ising_init_random": (_i32, [_vp, _u32, _u64, _vp]),
     "ising_energy": (_i32, [_vp, _u32, _vp, _vp]),
     "ising_accept_table": (_i32, [_dbl, _vp, _vp]),
@@ -148,6 +149,12 @@ def ising_sweep(h, d_spins, L: int, beta: float, n_sweeps: int, d_energy_trace=N
     _check(lib().ising_sweep(h, _ptr(d_spins), L, float(beta), n_sweeps, _ptr(d_energy_trace), _stream(cuda_stream)))
 
 
+def ising_sweep_multihit(h, d_spins, L: int, beta: float, n_sweeps: int, tile: int, k_hits: int, d_energy_trace=None,
+                         cuda_stream=None) -> None:
+    _check(lib().ising_sweep_multihit(h, _ptr(d_spins), L, float(beta), n_sweeps, tile, k_hits, _ptr(d_energy_trace),
+                                      _stream(cuda_stream)))
+
+
 def ising_init_random(d_spins, L: int, seed: int, cuda_stream=None) -> None:
     _check(lib().ising_init_random(_ptr(d_spins), L, seed & (2**64 - 1), _stream(cuda_stream)))
 
@@ -255,6 +262,9 @@ class Rng:
 
     def ising_sweep(self, d_spins, L, beta, n_sweeps, d_energy_trace=None, stream=None):
         ising_sweep(self._h, d_spins, L, beta, n_sweeps, d_energy_trace, stream)
+
+    def ising_sweep_multihit(self, d_spins, L, beta, n_sweeps, tile, k_hits, d_energy_trace=None, stream=None):
+        ising_sweep_multihit(self._h, d_spins, L, beta, n_sweeps, tile, k_hits, d_energy_trace, stream)
 
     def fill_u32_host(self, h_out, n, stream=None):
         rng_fill_u32_host(self._h, h_out, n, stream)

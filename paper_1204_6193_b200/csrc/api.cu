@@ -242,6 +242,37 @@ int ising_sweep(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_
     return RNG_OK;
 }
 
+int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_t n_sweeps, uint32_t tile,
+                         uint32_t k_hits, int64_t *d_trace, void *stream)
+{
+    if (!h) return fail(RNG_E_INVAL, "ising_sweep_multihit: handle is NULL");
+    if (!d_spins) return fail(RNG_E_INVAL, "ising_sweep_multihit: d_spins is NULL");
+    if (!aligned(d_spins, 16)) return fail(RNG_E_INVAL, "ising_sweep_multihit: d_spins must be 16-byte aligned");
+    if (!(beta == beta)) return fail(RNG_E_INVAL, "ising_sweep_multihit: beta is NaN");
+    if (tile < 2 || (tile & 1u) || tile > 44u || L < 2 * tile || L % tile || ((L / tile) & 1u))
+        return fail(RNG_E_INVAL, "ising_sweep_multihit: tile must be even, 2..44, divide L, with L/tile even");
+    if (k_hits < 1) return fail(RNG_E_INVAL, "ising_sweep_multihit: k_hits must be >= 1");
+    if (h->g.S != (uint64_t)L * L / 4) return fail(RNG_E_INVAL, "ising_sweep_multihit: needs n_streams == L*L/4");
+    if (h->g.kind == RNG_XS1024W && (tile * tile / 2u) % 32u)
+        return fail(RNG_E_INVAL, "ising_sweep_multihit: this kind needs whole warps per tile (tile a multiple of 8)");
+    const uint64_t per_sweep = 4ull * k_hits;
+    if (mul_overflows(per_sweep, n_sweeps) || h->g.draws_done + per_sweep * n_sweeps < h->g.draws_done)
+        return fail(RNG_E_INVAL, "ising_sweep_multihit: draw counter would overflow");
+    IsingTable tab;
+    ising_accept_table(beta, nullptr, tab.T);
+    cudaStream_t st = (cudaStream_t)stream;
+    uint64_t d = h->g.draws_done;
+    for (uint32_t t = 0; t < n_sweeps; t++) {
+        for (int c = 0; c < 2; c++) {
+            CU(launch_ising_multihit(*h, d_spins, L, tab, tile, k_hits, d, c, st));
+            d += 2ull * k_hits;
+        }
+        if (d_trace) CU(launch_ising_energy(d_spins, L, d_trace + t, st));
+    }
+    h->g.draws_done = d;
+    return RNG_OK;
+}
+
 int ising_init_random(int8_t *d_spins, uint32_t L, uint64_t seed, void *stream)
 {
     if (!d_spins || L < 2 || !aligned(d_spins, 16)) return fail(RNG_E_INVAL, "ising_init_random: bad arguments");

@@ -94,6 +94,9 @@ cudaError_t launch_ising_ms_unpack(int8_t *d_spins, const uint32_t *planes, uint
 cudaError_t launch_ising_ms_energy(const uint32_t *planes, uint32_t L, int64_t *d_out, cudaStream_t st);
 cudaError_t launch_ising_ms_half_sweep(const rng_handle &h, uint32_t *planes, uint32_t L, const IsingTable &tab, uint64_t K,
                                        uint64_t draws_done, int colour, cudaStream_t st);
+// ising_mh.cu (the paper's double-checkerboard multi-hit kernel; one launch per coarse colour)
+cudaError_t launch_ising_multihit(const rng_handle &h, int8_t *d_spins, uint32_t L, const IsingTable &tab, uint32_t T,
+                                  uint32_t k_hits, uint64_t draws_done, int coarse, cudaStream_t st);
 cudaError_t launch_ising_init_random(int8_t *d_spins, uint32_t L, uint64_t seed, cudaStream_t st);
 cudaError_t launch_ising_energy(const int8_t *d_spins, uint32_t L, int64_t *d_out, cudaStream_t st);
 

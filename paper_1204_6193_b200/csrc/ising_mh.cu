@@ -1,0 +1,108 @@
+// ising_mh.cu -- the paper's own consumer kernel: double-checkerboard Metropolis with multi-hit
+// updates (PAPER.md:56 "a double checkerboard decomposition", :58 "updating the spins of a tile
+// once (k = 1) ... two random numbers are produced per state load and save operation ... multi-hit
+// updates (k = 100), 200 random numbers are produced per access to global memory"; the kernel is
+// described in Refs.[13,25], the order used here is reading R-E9 of DESIGN.md).
+//
+//   The lattice is cut into T x T tiles; tile (tx, ty) has coarse colour (tx+ty)&1.  A sweep is
+//   coarse colour 0, then 1; one launch per coarse colour, one CTA of T*T/2 threads per tile of that
+//   colour.  The CTA loads its tile and the one-site halo around it into shared memory (the halo
+//   belongs to resting tiles of the other coarse colour), every thread loads ITS generator state
+//   once, and the tile receives k hits: a hit = all sites of fine colour 0, barrier, all sites of
+//   fine colour 1, barrier.  Thread t owns the horizontal domino (2 xh, 2 xh + 1) of row y_l,
+//   t = y_l T/2 + xh, i.e. one site of each fine colour, and keeps both spins in registers; the
+//   three foreign neighbours of a site come from shared memory.  Stream s = p T*T/2 + t for tile
+//   number p = ty (L/T/2) + txh of either coarse colour (S = L*L/4 streams, one per thread, as in the
+//   paper: 1024^2 sites <-> 262144 threads); a stream spends its draws in the order
+//   (coarse colour, hit, fine colour).  2k draws per state load: the paper's k = 1 and k = 100
+//   columns of Table 1 are this kernel with k_hits = 1 and 100.
+// Acceptance as everywhere: flip iff (r >> 8) < T[(h+4)/2]  (exactly (float)(r>>8) 2^-24 < P).
+// Product code (sm_100a); shares nothing with oracle/.
+#include "internal.h"
+#include "streams.cuh"
+
+namespace rngb200 {
+
+template <int KIND>
+__global__ void ising_multihit_kernel(Gen g, int8_t *__restrict__ sp, uint32_t L, IsingTable tab, uint32_t T,
+                                      uint32_t k_hits, uint32_t C)
+{
+    extern __shared__ __align__(16) int8_t tile[]; // (T+2) rows of RS bytes; interior row y_l at row y_l+1, col 4..
+    const uint32_t RS = T + 8u, half = T >> 1;
+    const uint32_t t = threadIdx.x;
+    const uint32_t nth = (L / T) >> 1;
+    const uint32_t p = blockIdx.x;
+    const uint32_t ty = p / nth, txh = p - ty * nth;
+    const uint32_t tx = 2u * txh + ((ty + C) & 1u);
+    const uint32_t x0 = tx * T, y0 = ty * T; // tile origin (both even: local parity = global parity)
+    const uint32_t yl = t / half, xh = t - yl * half;
+
+    // ---- load: own domino (also kept in registers), then the halo by the first T threads ----
+    int8_t *grow = sp + (uint64_t)(y0 + yl) * L + x0 + 2u * xh;
+    const uint16_t dom = *reinterpret_cast<const uint16_t *>(grow);
+    int8_t *mine = tile + (yl + 1u) * RS + 4u + 2u * xh;
+    *reinterpret_cast<uint16_t *>(mine) = dom;
+    if (t < T) {
+        const uint32_t yu = y0 ? y0 - 1u : L - 1u, yd = (y0 + T == L) ? 0u : y0 + T;
+        const uint32_t xl = x0 ? x0 - 1u : L - 1u, xr = (x0 + T == L) ? 0u : x0 + T;
+        tile[0u * RS + 4u + t] = sp[(uint64_t)yu * L + x0 + t];
+        tile[(T + 1u) * RS + 4u + t] = sp[(uint64_t)yd * L + x0 + t];
+        tile[(t + 1u) * RS + 3u] = sp[(uint64_t)(y0 + t) * L + xl];
+        tile[(t + 1u) * RS + 4u + T] = sp[(uint64_t)(y0 + t) * L + xr];
+    }
+    const uint64_t s = (uint64_t)p * (half * T) + t;
+    Stream<KIND> gen;
+    gen.load(g, s);
+    __syncthreads();
+
+    // fine colour c site of the domino: x_l = 2 xh + ((y_l + c) & 1)
+    const uint32_t par = yl & 1u;       // colour-0 site is byte `par` of the domino, colour-1 site byte 1-par
+    int sa = (int)(int8_t)(par ? (dom >> 8) : (dom & 0xff));  // colour 0
+    int sb = (int)(int8_t)(par ? (dom & 0xff) : (dom >> 8));  // colour 1
+    int8_t *pa = mine + par, *pb = mine + (1u - par);
+    // foreign horizontal neighbour: the site beyond the domino on the side away from the partner
+    const int da = par ? 1 : -1; // colour-0 site at byte par: partner on the other side
+    for (uint32_t hit = 0; hit < k_hits; hit++) {
+        {
+            const int nn = sb + (int)pa[da] + (int)pa[-(int)RS] + (int)pa[RS];
+            const int h = sa * nn;
+            const uint32_t r = gen.next();
+            if ((r >> 8) < tab.T[(h + 4) >> 1]) {
+                sa = -sa;
+                *pa = (int8_t)sa;
+            }
+        }
+        __syncthreads();
+        {
+            const int nn = sa + (int)pb[-da] + (int)pb[-(int)RS] + (int)pb[RS];
+            const int h = sb * nn;
+            const uint32_t r = gen.next();
+            if ((r >> 8) < tab.T[(h + 4) >> 1]) {
+                sb = -sb;
+                *pb = (int8_t)sb;
+            }
+        }
+        __syncthreads();
+    }
+    gen.store(g, s);
+    const uint32_t lo = (uint32_t)(uint8_t)(par ? sb : sa), hi = (uint32_t)(uint8_t)(par ? sa : sb);
+    *reinterpret_cast<uint16_t *>(grow) = (uint16_t)(lo | (hi << 8));
+}
+
+cudaError_t launch_ising_multihit(const rng_handle &h, int8_t *d_spins, uint32_t L, const IsingTable &tab, uint32_t T,
+                                  uint32_t k_hits, uint64_t draws_done, int coarse, cudaStream_t st)
+{
+    Gen g = h.g;
+    g.draws_done = draws_done;
+    const uint32_t threads = T * T / 2u;
+    const uint32_t tiles = (L / T) * (L / T) / 2u;
+    const size_t smem = (size_t)(T + 2u) * (T + 8u);
+#define MH(KIND) \
+    ising_multihit_kernel<KIND><<<tiles, threads, smem, st>>>(g, d_spins, L, tab, T, k_hits, (uint32_t)coarse)
+    RNGB200_DISPATCH_KIND(g.kind, MH)
+#undef MH
+    count_launch();
+    return cudaGetLastError();
+}
+
+} // namespace rngb200

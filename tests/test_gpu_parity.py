@@ -516,3 +516,67 @@ def test_xs1024_skip_seeding_large_shard_against_the_skip_matrix():
     for i in (0, 1, 2, 3, 63, 64, 1023, 1024, 2047, 2048, 2999):
         assert np.array_equal(st[i], inst(G0 + i)), i
     assert len({st[i].tobytes() for i in range(n_inst)}) == n_inst
+
+
+# ---------------------------------------------------------------------------------
+# the paper's own consumer: double checkerboard with multi-hit updates (R-E9)
+# ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("L,T,k,sweeps", [(4, 2, 1, 6), (8, 2, 3, 4), (16, 8, 1, 5), (32, 8, 7, 3), (64, 16, 2, 4),
+                                          (128, 32, 5, 2), (96, 16, 100, 1), (80, 20, 3, 2), (176, 44, 2, 2)])
+def test_ising_multihit_bit_exact(kind, L, T, k, sweeps):
+    S = L * L // 4
+    if kind in XS_KINDS and (S % 32 or (T * T // 2) % 32):
+        pytest.skip("whole warp instances per tile only")
+    beta = 0.44068679350977147
+    g, o = pkg.Rng(kind, S, 13), oracle.Rng(kind, S, 13)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, 4)
+    sp_o = oracle.ising_init_random(L, 4)
+    tr = torch.empty(sweeps, dtype=torch.int64, device="cuda")
+    g.ising_sweep_multihit(sp, L, beta, sweeps, T, k, tr)
+    tr_o = o.ising_sweep_multihit(sp_o, L, beta, sweeps, T, k, trace=True)
+    assert np.array_equal(sp.cpu().numpy(), sp_o)
+    assert np.array_equal(tr.cpu().numpy(), tr_o)
+    assert g.draws_done == o.draws_done == 4 * k * sweeps
+    # the streams continue: a plain fill afterwards gives the oracle's next draws
+    out = dev_u32(S * 5)
+    g.fill_u32(out, 5)
+    assert np.array_equal(host(out, S * 5), o.fill_u32(5))
+    g.close()
+
+
+def test_ising_multihit_argument_errors():
+    g = pkg.Rng(pkg.RNG_PHILOX4X32_10, 16, 1)
+    sp = torch.ones(64, dtype=torch.int8, device="cuda")
+    for L, T, k in ((8, 3, 1), (8, 8, 1), (8, 2, 0), (8, 46, 1)):
+        with pytest.raises(pkg.RngError) as e:
+            g.ising_sweep_multihit(sp, L, 0.3, 1, T, k)
+        assert e.value.code == pkg.RNG_E_INVAL
+    g.close()
+    g = pkg.Rng(pkg.RNG_PHILOX4X32_10, 32, 1)          # needs L*L/4 = 16 streams
+    with pytest.raises(pkg.RngError):
+        g.ising_sweep_multihit(sp, 8, 0.3, 1, 2, 1)
+    g.close()
+
+
+@pytest.mark.parametrize("kind", [pkg.RNG_PHILOX4X32_10, pkg.RNG_XORWOW, pkg.RNG_XS1024W_SKIP],
+                         ids=["philox10", "xorwow", "xs1024w_skip"])
+def test_table1_multihit_L1024_beta04_energy_within_3_sigma(kind):
+    """the paper's application test with its own kernel shape (Table 1): L = 1024, beta = 0.4,
+    double checkerboard, one stream per thread (262144), e and C_V against Kaufman's exact values"""
+    from exact_ising import kaufman
+    L, T, k, beta = 1024, 16, 1, 0.4
+    ex = kaufman(L, beta)
+    g = pkg.Rng(kind, L * L // 4, 1)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, 2)
+    g.ising_sweep_multihit(sp, L, beta, 3000, T, k)
+    n = 20000
+    tr = torch.empty(n, dtype=torch.int64, device="cuda")
+    g.ising_sweep_multihit(sp, L, beta, n, T, k, tr)
+    e = tr.cpu().numpy().astype(np.float64) / (L * L)
+    bins = e.reshape(-1, 500).mean(axis=1)
+    sigma = bins.std(ddof=1) / np.sqrt(len(bins))
+    assert abs(e.mean() - ex["e"]) < 3 * sigma, (e.mean(), ex["e"], sigma)
+    g.close()
