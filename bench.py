@@ -69,12 +69,12 @@ def issue_peak_tinst(sm_mhz: float) -> float:
 # shifts + 66 xors per 32 words (the zero padding drops 10 of 32 words per phase) + Weyl add (1)
 # + checksum (2)
 ALG_INST_PER_DRAW = {W.LCG64: 5.0, W.LCG64_LEAPFROG: 5.0, W.XORWOW: 10.0, W.PHILOX4X32_10: 12.0, W.XS1024W: 7.0,
-                     W.PHILOX4X32_7: 9.0, W.LCG32: 3.0}
+                     W.PHILOX4X32_7: 9.0, W.LCG32: 3.0, W.XS1024W_SKIP: 7.0}
 # multi-spin-coded update: two threshold compares of two instructions each + the bit-sliced
 # neighbour count / flip logic amortised over the 32 sites of a word (about 1), excl. the draw
 ALG_INST_PER_ISING_UPDATE = 5.0
 STATE_BYTES = {W.LCG64: 8, W.LCG64_LEAPFROG: 8, W.XORWOW: 24, W.PHILOX4X32_10: 0, W.XS1024W: 4, W.PHILOX4X32_7: 0,
-               W.LCG32: 4}
+               W.LCG32: 4, W.XS1024W_SKIP: 4}
 
 
 class ClockSampler:
@@ -245,19 +245,29 @@ class IsingJob(Job):
         pkg.ising_init_random(self.spins, cfg.L, cfg.lattice_seed + rank)
         # a half-sweep launch loads and stores every stream's state once: with few updates per
         # stream (the paper's k = 1 regime) that traffic, not the arithmetic, bounds the kernel
-        self.K = cfg.L * cfg.L // 2 // cfg.n_streams
+        self.K = cfg.L * cfg.L // 2 // cfg.n_streams if not cfg.tile else 2 * cfg.k_hits  # draws per state load
         self.state_bytes_per_update = 2.0 * STATE_BYTES[cfg.kind] / self.K
         if self.state_bytes_per_update >= 4.0:
             self.bound = "hbm"
 
     def units_per_step(self):
-        return float(self.cfg.L * self.cfg.L * self.sweeps)
+        return float(self.cfg.L * self.cfg.L * self.sweeps * self.cfg.k_hits)
 
     def step(self):
-        self.rng.ising_sweep(self.spins, self.cfg.L, self.cfg.beta, self.sweeps)
+        if self.cfg.tile:
+            self.rng.ising_sweep_multihit(self.spins, self.cfg.L, self.cfg.beta, self.sweeps, self.cfg.tile,
+                                          self.cfg.k_hits)
+        else:
+            self.rng.ising_sweep(self.spins, self.cfg.L, self.cfg.beta, self.sweeps)
 
     def alg_per_launch(self):
         k = self.cfg.L * self.cfg.L // 2  # updates per half-sweep launch
+        if self.cfg.tile:
+            # one launch = one coarse colour: half the sites, k_hits updates each; byte lattice, one generator
+            # state load + store per thread.  ~12 instructions per update on bytes in shared memory + the draw
+            if self.bound == "hbm":
+                return 2.0 * STATE_BYTES[self.cfg.kind] * self.cfg.n_streams + 2.0 * k
+            return (12.0 + ALG_INST_PER_DRAW[self.cfg.kind]) * k * self.cfg.k_hits
         if self.bound == "hbm":
             # state load + store per stream, plus the two bit planes read and one written (1 bit per site)
             return 2.0 * STATE_BYTES[self.cfg.kind] * self.cfg.n_streams + 3.0 * k / 8.0
@@ -347,6 +357,15 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
         "C5b_philox": lambda: IsingJob(W.C5B_PHILOX, rank, world, ising_sweeps),
         "C5b_xorwow": lambda: IsingJob(W.C5B_XORWOW, rank, world, ising_sweeps),
         "C5b_xorwow_K8": lambda: IsingJob(W.C5B_XORWOW_K8, rank, world, ising_sweeps),
+        "T1_xorwow_k1": lambda: IsingJob(W.T1_XORWOW_K1, rank, world, W.T1_XORWOW_K1.n_sweeps),
+        "T1_xorwow_k100": lambda: IsingJob(W.T1_XORWOW_K100, rank, world, W.T1_XORWOW_K100.n_sweeps),
+        "T1_philox_k100": lambda: IsingJob(W.T1_PHILOX_K100, rank, world, W.T1_PHILOX_K100.n_sweeps),
+        "T1_xs1024skip_k100": lambda: IsingJob(W.T1_XS1024_K100, rank, world, W.T1_XS1024_K100.n_sweeps),
+        "T1_lcg32_k100": lambda: IsingJob(W.T1_LCG32_K100, rank, world, W.T1_LCG32_K100.n_sweeps),
+        "T1big_xorwow_k100": lambda: IsingJob(W.T1BIG_XORWOW_K100, rank, world, W.T1BIG_XORWOW_K100.n_sweeps),
+        "T1big_xorwow_k1": lambda: IsingJob(W.T1BIG_XORWOW_K1, rank, world, W.T1BIG_XORWOW_K1.n_sweeps),
+        "T1big_xorwow_k100_t8": lambda: IsingJob(W.T1BIG_XORWOW_K100_T8, rank, world, W.T1BIG_XORWOW_K100_T8.n_sweeps),
+        "T1_xorwow_k100_t8": lambda: IsingJob(W.T1_XORWOW_K100_T8, rank, world, W.T1_XORWOW_K100_T8.n_sweeps),
     }
     if name not in table:
         raise SystemExit(f"unknown --workload {name}; choose from {sorted(table)}")
@@ -360,7 +379,10 @@ SUITE = [("C2_f32", 20, 3), ("C1_u32", 200, 10), ("C1_f32", 200, 10), ("C1big_u3
          ("C5b_xorwow_K8", 1, 1),
          ("N1_philox7_u32", 20, 3), ("N1_lcg32_u32", 20, 3), ("N1_philox7_draw", 20, 3), ("N1_philox10_draw", 20, 3),
          ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3),
-         ("N2_seed_xs1024_random", 5, 3), ("N2_seed_xs1024_skip", 5, 3)]
+         ("N2_seed_xs1024_random", 5, 3), ("N2_seed_xs1024_skip", 5, 3),
+         ("T1_xorwow_k1", 3, 3), ("T1_xorwow_k100", 3, 3), ("T1_philox_k100", 3, 3), ("T1_xs1024skip_k100", 3, 3),
+         ("T1_lcg32_k100", 3, 3), ("T1big_xorwow_k100", 3, 3), ("T1big_xorwow_k1", 3, 3),
+         ("T1_xorwow_k100_t8", 3, 3), ("T1big_xorwow_k100_t8", 3, 3)]
 
 
 # ------------------------------------------------------------------------------------
@@ -372,6 +394,23 @@ def oracle_sample_rate(workload: str, target_s: float = 4.0) -> dict:
     import numpy as np
     import oracle
     cores = oracle.threads()
+    if workload.startswith("T1"):
+        cfg = {"T1_xorwow_k1": W.T1_XORWOW_K1, "T1_xorwow_k100": W.T1_XORWOW_K100, "T1_philox_k100": W.T1_PHILOX_K100,
+               "T1_xs1024skip_k100": W.T1_XS1024_K100, "T1_lcg32_k100": W.T1_LCG32_K100,
+               "T1big_xorwow_k100": W.T1BIG_XORWOW_K100, "T1big_xorwow_k1": W.T1BIG_XORWOW_K1,
+               "T1big_xorwow_k100_t8": W.T1BIG_XORWOW_K100_T8, "T1_xorwow_k100_t8": W.T1_XORWOW_K100_T8}[workload]
+        L = 1024  # the paper's lattice; for the L = 8192 workloads 1/64 of the area, same tile and hits
+        sp = oracle.ising_init_random(L, cfg.lattice_seed)
+        r = oracle.Rng(cfg.kind, L * L // 4, cfg.seed)
+        sweeps, t0 = 0, time.perf_counter()
+        while True:
+            r.ising_sweep_multihit(sp, L, cfg.beta, 1, cfg.tile, cfg.k_hits)
+            sweeps += 1
+            dt = time.perf_counter() - t0
+            if dt > target_s or sweeps >= 1000:
+                break
+        return {"value": L * L * sweeps * cfg.k_hits / dt / 1e9, "unit": "flips/ns", "cores": cores, "kind": "oracle",
+                "sample": f"L={L}, tile {cfg.tile}, k={cfg.k_hits}, {sweeps} sweeps", "seconds": dt}
     if workload.startswith("C5b"):
         cfg = {"C5b_philox": W.C5B_PHILOX, "C5b_xorwow": W.C5B_XORWOW, "C5b_xorwow_K8": W.C5B_XORWOW_K8}[workload]
         L = 2048  # 1/16 of the lattice area, same K per stream
@@ -575,7 +614,7 @@ def main():
             "data": "synthetic (seeded streams; this path has no dataset)",
             "config": {"workload": res["name"], "l2": "4 GiB output per step, larger than the 126 MB L2"
                        if not isinstance(job, IsingJob) else "64 MiB lattice is L2-resident by design (DESIGN.md s7)",
-                       "streams_per_gpu": getattr(job.cfg, "n_streams", None), "parallelism": f"streams x{world}"},
+                       "streams_per_gpu": getattr(getattr(job, "cfg", None), "n_streams", getattr(job, "n_local", None)), "parallelism": f"streams x{world}"},
             "clocks": res.get("clocks"), "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],
         }
         if e2e:

@@ -23,15 +23,27 @@
 
 namespace rngb200 {
 
-template <int KIND>
+// WARP_TILE: tile = 8, a tile is exactly one warp (32 dominoes): a CTA hosts blockDim.x/32 tiles, each in
+// its own slab of shared memory, and the two barriers of a hit are __syncwarp() instead of __syncthreads().
+template <int KIND, bool WARP_TILE>
 __global__ void ising_multihit_kernel(Gen g, int8_t *__restrict__ sp, uint32_t L, IsingTable tab, uint32_t T,
-                                      uint32_t k_hits, uint32_t C)
+                                      uint32_t k_hits, uint32_t C, uint32_t n_tiles)
 {
-    extern __shared__ __align__(16) int8_t tile[]; // (T+2) rows of RS bytes; interior row y_l at row y_l+1, col 4..
+    extern __shared__ __align__(16) int8_t mh_smem[]; // 16 words of thresholds, then the tile slab(s)
+    // thresholds indexed by h + 4 (h = spin * neighbour sum, even): word address = 4 h + const, one IMAD
+    uint32_t *thr = reinterpret_cast<uint32_t *>(mh_smem);
+    for (uint32_t i = threadIdx.x; i < 5u; i += blockDim.x) thr[2u * i] = tab.T[i]; // a 2 x 2 tile has 2 threads
     const uint32_t RS = T + 8u, half = T >> 1;
-    const uint32_t t = threadIdx.x;
+    // (T+2) rows of RS bytes; interior row y_l at row y_l+1, columns 4 .. 4+T-1, halo columns 3 and 4+T
+    int8_t *tile = mh_smem + 64 + (WARP_TILE ? (threadIdx.x >> 5) * (((T + 2u) * RS + 15u) & ~15u) : 0u);
+    const uint32_t t = WARP_TILE ? (threadIdx.x & 31u) : threadIdx.x;
     const uint32_t nth = (L / T) >> 1;
-    const uint32_t p = blockIdx.x;
+    const uint32_t p = WARP_TILE ? blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5) : blockIdx.x;
+    const bool tile_live = p < n_tiles; // warp-uniform; dead warps still take part in the CTA barrier below
+    if (WARP_TILE && !tile_live) {
+        __syncthreads();
+        return;
+    }
     const uint32_t ty = p / nth, txh = p - ty * nth;
     const uint32_t tx = 2u * txh + ((ty + C) & 1u);
     const uint32_t x0 = tx * T, y0 = ty * T; // tile origin (both even: local parity = global parity)
@@ -53,36 +65,41 @@ __global__ void ising_multihit_kernel(Gen g, int8_t *__restrict__ sp, uint32_t L
     const uint64_t s = (uint64_t)p * (half * T) + t;
     Stream<KIND> gen;
     gen.load(g, s);
-    __syncthreads();
+    __syncthreads(); // thresholds and tile(s) are in place
+    auto hit_barrier = [&]() {
+        if constexpr (WARP_TILE) __syncwarp();
+        else __syncthreads();
+    };
 
     // fine colour c site of the domino: x_l = 2 xh + ((y_l + c) & 1)
     const uint32_t par = yl & 1u;       // colour-0 site is byte `par` of the domino, colour-1 site byte 1-par
     int sa = (int)(int8_t)(par ? (dom >> 8) : (dom & 0xff));  // colour 0
     int sb = (int)(int8_t)(par ? (dom & 0xff) : (dom >> 8));  // colour 1
+    const char *thr4 = reinterpret_cast<const char *>(thr) + 16; // + 4 h
     int8_t *pa = mine + par, *pb = mine + (1u - par);
     // foreign horizontal neighbour: the site beyond the domino on the side away from the partner
     const int da = par ? 1 : -1; // colour-0 site at byte par: partner on the other side
     for (uint32_t hit = 0; hit < k_hits; hit++) {
         {
             const int nn = sb + (int)pa[da] + (int)pa[-(int)RS] + (int)pa[RS];
-            const int h = sa * nn;
+            const uint32_t th = *reinterpret_cast<const uint32_t *>(thr4 + 4 * sa * nn);
             const uint32_t r = gen.next();
-            if ((r >> 8) < tab.T[(h + 4) >> 1]) {
+            if ((r >> 8) < th) {
                 sa = -sa;
                 *pa = (int8_t)sa;
             }
         }
-        __syncthreads();
+        hit_barrier();
         {
             const int nn = sa + (int)pb[-da] + (int)pb[-(int)RS] + (int)pb[RS];
-            const int h = sb * nn;
+            const uint32_t th = *reinterpret_cast<const uint32_t *>(thr4 + 4 * sb * nn);
             const uint32_t r = gen.next();
-            if ((r >> 8) < tab.T[(h + 4) >> 1]) {
+            if ((r >> 8) < th) {
                 sb = -sb;
                 *pb = (int8_t)sb;
             }
         }
-        __syncthreads();
+        hit_barrier();
     }
     gen.store(g, s);
     const uint32_t lo = (uint32_t)(uint8_t)(par ? sb : sa), hi = (uint32_t)(uint8_t)(par ? sa : sb);
@@ -94,13 +111,22 @@ cudaError_t launch_ising_multihit(const rng_handle &h, int8_t *d_spins, uint32_t
 {
     Gen g = h.g;
     g.draws_done = draws_done;
-    const uint32_t threads = T * T / 2u;
     const uint32_t tiles = (L / T) * (L / T) / 2u;
-    const size_t smem = (size_t)(T + 2u) * (T + 8u);
-#define MH(KIND) \
-    ising_multihit_kernel<KIND><<<tiles, threads, smem, st>>>(g, d_spins, L, tab, T, k_hits, (uint32_t)coarse)
-    RNGB200_DISPATCH_KIND(g.kind, MH)
+    const size_t slab = ((size_t)(T + 2u) * (T + 8u) + 15u) & ~(size_t)15u;
+    if (T == 8u) { // one warp per tile, four tiles per CTA
+        const uint32_t wpc = 4u, grid = (tiles + wpc - 1u) / wpc;
+#define MH(KIND)                                                                                                  \
+    ising_multihit_kernel<KIND, true><<<grid, wpc * 32u, 64 + wpc * slab, st>>>(g, d_spins, L, tab, T, k_hits, \
+                                                                                 (uint32_t)coarse, tiles)
+        RNGB200_DISPATCH_KIND(g.kind, MH)
 #undef MH
+    } else {
+#define MH(KIND)                                                                                               \
+    ising_multihit_kernel<KIND, false><<<tiles, T * T / 2u, 64 + slab, st>>>(g, d_spins, L, tab, T, k_hits, \
+                                                                              (uint32_t)coarse, tiles)
+        RNGB200_DISPATCH_KIND(g.kind, MH)
+#undef MH
+    }
     count_launch();
     return cudaGetLastError();
 }

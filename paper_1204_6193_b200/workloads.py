@@ -39,6 +39,8 @@ class IsingCfg:
     n_sweeps: int
     seed: int = MASTER_SEED
     lattice_seed: int = LATTICE_SEED
+    tile: int = 0              # > 0: the paper's double-checkerboard multi-hit kernel with this tile size
+    k_hits: int = 1            # hits per tile visit (k = 1 and k = 100)
 
 
 # C1: 64-bit LCG, 1024 streams x 4096 u32 (16 MiB) -- the small case the oracle does in ms
@@ -69,6 +71,18 @@ C5A_XORWOW = IsingCfg("C5a_ising_L4_xorwow", XORWOW, 4, 0.3, 8, 1000)
 C5B_PHILOX = IsingCfg("C5b_ising_L8192_philox_K4", PHILOX4X32_10, 8192, BETA_C, 1 << 23, 1000)
 C5B_XORWOW = IsingCfg("C5b_ising_L8192_xorwow_K256", XORWOW, 8192, BETA_C, 1 << 17, 1000)
 C5B_XORWOW_K8 = IsingCfg("C5b_ising_L8192_xorwow_K8", XORWOW, 8192, BETA_C, 1 << 22, 1000)
+
+# the paper's Table 1 workload: 1024^2 at beta = 0.4, double checkerboard,
+# one stream per thread (262144), k = 1 and k = 100 hits; and the same at L = 8192 (2^24 streams) to fill a B200
+T1_XORWOW_K1 = IsingCfg("T1_multihit_L1024_xorwow_k1", XORWOW, 1024, 0.4, 1 << 18, 1000, tile=16, k_hits=1)
+T1_XORWOW_K100 = IsingCfg("T1_multihit_L1024_xorwow_k100", XORWOW, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
+T1_PHILOX_K100 = IsingCfg("T1_multihit_L1024_philox_k100", PHILOX4X32_10, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
+T1_XS1024_K100 = IsingCfg("T1_multihit_L1024_xs1024skip_k100", XS1024W_SKIP, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
+T1_LCG32_K100 = IsingCfg("T1_multihit_L1024_lcg32_k100", LCG32, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
+T1BIG_XORWOW_K100 = IsingCfg("T1big_multihit_L8192_xorwow_k100", XORWOW, 8192, 0.4, 1 << 24, 2, tile=16, k_hits=100)
+T1BIG_XORWOW_K1 = IsingCfg("T1big_multihit_L8192_xorwow_k1", XORWOW, 8192, 0.4, 1 << 24, 100, tile=16, k_hits=1)
+T1BIG_XORWOW_K100_T8 = IsingCfg("T1big_multihit_L8192_xorwow_k100_tile8", XORWOW, 8192, 0.4, 1 << 24, 2, tile=8, k_hits=100)
+T1_XORWOW_K100_T8 = IsingCfg("T1_multihit_L1024_xorwow_k100_tile8", XORWOW, 1024, 0.4, 1 << 18, 10, tile=8, k_hits=100)
 
 FILL_CONFIGS = [C1, C2, C3_FILL, C1_BIG, C4_FILL]
 DRAW_CONFIGS = [C3, C4_DRAW]
