@@ -77,6 +77,25 @@ STATE_BYTES = {W.LCG64: 8, W.LCG64_LEAPFROG: 8, W.XORWOW: 24, W.PHILOX4X32_10: 0
                W.LCG32: 4, W.XS1024W_SKIP: 4}
 
 
+# The paper's own numbers (GTX 480) for the workloads that have one: context, not a target.
+# Table 2: peak 10^9 numbers/s consumed in-register; Table 1: 1/t_up flips/ns
+# of the double-checkerboard code at L = 1024, beta = 0.4.
+PAPER_GTX480 = {
+    "C3_xorwow_2^22x256_draw_reduce": (19.0, "Gnum/s", "PAPER.md:266"),
+    "C4_xs1024_2^24x4096_draw_draw_reduce": (18.0, "Gnum/s", "PAPER.md:268"),
+    "N1_philox10_2^22x256_draw_reduce": (30.0, "Gnum/s", "PAPER.md:270"),
+    "N1_philox7_2^22x256_draw_reduce": (41.0, "Gnum/s", "PAPER.md:269"),
+    "N1_lcg64_2^22x256_draw_reduce": (46.0, "Gnum/s", "PAPER.md:261"),
+    "N1_lcg32_2^22x256_draw_reduce": (58.0, "Gnum/s", "PAPER.md:259"),
+    "T1_multihit_L1024_xorwow_k1": (1.0 / 0.7956, "flips/ns", "PAPER.md:88"),
+    "T1_multihit_L1024_xorwow_k100": (1.0 / 0.0576, "flips/ns", "PAPER.md:88"),
+    "T1_multihit_L1024_xorwow_k100_tile8": (1.0 / 0.0576, "flips/ns", "PAPER.md:88"),
+    "T1_multihit_L1024_philox_k100": (1.0 / 0.0622, "flips/ns", "PAPER.md:91"),
+    "T1_multihit_L1024_xs1024skip_k100": (1.0 / 0.0721, "flips/ns", "PAPER.md:89"),
+    "T1_multihit_L1024_lcg32_k100": (1.0 / 0.0402, "flips/ns", "PAPER.md:80"),
+}
+
+
 class ClockSampler:
     """samples SM clock and throttle reasons with NVML while the timed region runs"""
 
@@ -329,6 +348,10 @@ def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, 
                            "peak_source": "148 SM x 4 SMSP x 32 lanes x sm_max_mhz (issue slots; DESIGN.md s7)"}
     if clocks:
         res["clocks"] = clocks
+    if job.name in PAPER_GTX480:
+        v, u, cite = PAPER_GTX480[job.name]
+        res["paper_gtx480"] = {"value": v, "unit": u, "cite": cite, "ratio": value / v,
+                               "note": "the paper's number on its GTX 480: context, not the target"}
     return res
 
 
@@ -610,13 +633,15 @@ def main():
         line = {
             "metric": METRIC, "value": res["value"], "unit": res["unit"], "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": res["dtype"],
+            "vs_baseline": res["paper_gtx480"]["ratio"] if "paper_gtx480" in res else None, "dtype": res["dtype"],
             "data": "synthetic (seeded streams; this path has no dataset)",
             "config": {"workload": res["name"], "l2": "4 GiB output per step, larger than the 126 MB L2"
                        if not isinstance(job, IsingJob) else "64 MiB lattice is L2-resident by design (DESIGN.md s7)",
                        "streams_per_gpu": getattr(getattr(job, "cfg", None), "n_streams", getattr(job, "n_local", None)), "parallelism": f"streams x{world}"},
             "clocks": res.get("clocks"), "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],
         }
+        if "paper_gtx480" in res:
+            line["paper_gtx480"] = res["paper_gtx480"]
         if e2e:
             line["e2e"] = e2e
         if cpu:
