@@ -69,12 +69,13 @@ def issue_peak_tinst(sm_mhz: float) -> float:
 # shifts + 66 xors per 32 words (the zero padding drops 10 of 32 words per phase) + Weyl add (1)
 # + checksum (2)
 ALG_INST_PER_DRAW = {W.LCG64: 5.0, W.LCG64_LEAPFROG: 5.0, W.XORWOW: 10.0, W.PHILOX4X32_10: 12.0, W.XS1024W: 7.0,
-                     W.PHILOX4X32_7: 9.0, W.LCG32: 3.0, W.XS1024W_SKIP: 7.0}
+                     W.PHILOX4X32_7: 9.0, W.LCG32: 3.0, W.XS1024W_SKIP: 7.0,
+                     W.LCG64_BOTH: 3.5}
 # multi-spin-coded update: two threshold compares of two instructions each + the bit-sliced
 # neighbour count / flip logic amortised over the 32 sites of a word (about 1), excl. the draw
 ALG_INST_PER_ISING_UPDATE = 5.0
 STATE_BYTES = {W.LCG64: 8, W.LCG64_LEAPFROG: 8, W.XORWOW: 24, W.PHILOX4X32_10: 0, W.XS1024W: 4, W.PHILOX4X32_7: 0,
-               W.LCG32: 4, W.XS1024W_SKIP: 4}
+               W.LCG32: 4, W.XS1024W_SKIP: 4, W.LCG64_BOTH: 8}
 
 
 # The paper's own numbers (GTX 480) for the workloads that have one: context, not a target.
@@ -372,6 +373,8 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
         "N1_philox10_draw": lambda: DrawJob(W.N1_PHILOX10_DRAW, rank, world, buf),
         "N1_lcg32_draw": lambda: DrawJob(W.N1_LCG32_DRAW, rank, world, buf),
         "N1_lcg64_draw": lambda: DrawJob(W.N1_LCG64_DRAW, rank, world, buf),
+        "N1_lcg64both_draw": lambda: DrawJob(W.N1_LCG64BOTH_DRAW, rank, world, buf),
+        "N1_lcg64both_u32": lambda: FillJob(W.N1_LCG64BOTH, False, rank, world, buf),
         "C3_draw": lambda: DrawJob(W.C3, rank, world, buf),
         "C4_fill": lambda: FillJob(W.C4_FILL, False, rank, world, buf),
         "C4_draw": lambda: DrawJob(W.C4_DRAW, rank, world, buf),
@@ -401,7 +404,7 @@ SUITE = [("C2_f32", 20, 3), ("C1_u32", 200, 10), ("C1_f32", 200, 10), ("C1big_u3
          ("C3_draw", 20, 3), ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1),
          ("C5b_xorwow_K8", 1, 1),
          ("N1_philox7_u32", 20, 3), ("N1_lcg32_u32", 20, 3), ("N1_philox7_draw", 20, 3), ("N1_philox10_draw", 20, 3),
-         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3),
+         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3), ("N1_lcg64both_draw", 20, 3), ("N1_lcg64both_u32", 20, 3),
          ("N2_seed_xs1024_random", 5, 3), ("N2_seed_xs1024_skip", 5, 3),
          ("T1_xorwow_k1", 3, 3), ("T1_xorwow_k100", 3, 3), ("T1_philox_k100", 3, 3), ("T1_xs1024skip_k100", 3, 3),
          ("T1_lcg32_k100", 3, 3), ("T1big_xorwow_k100", 3, 3), ("T1big_xorwow_k1", 3, 3),
@@ -454,7 +457,8 @@ def oracle_sample_rate(workload: str, target_s: float = 4.0) -> dict:
             "C3_draw": (W.C3, "draw_reduce"), "C4_fill": (W.C4_FILL, "fill_u32"), "C4_draw": (W.C4_DRAW, "draw_reduce"),
             "N1_philox7_u32": (W.N1_PHILOX7, "fill_u32"), "N1_lcg32_u32": (W.N1_LCG32, "fill_u32"),
             "N1_philox7_draw": (W.N1_PHILOX7_DRAW, "draw_reduce"), "N1_philox10_draw": (W.N1_PHILOX10_DRAW, "draw_reduce"),
-            "N1_lcg32_draw": (W.N1_LCG32_DRAW, "draw_reduce"), "N1_lcg64_draw": (W.N1_LCG64_DRAW, "draw_reduce")}
+            "N1_lcg32_draw": (W.N1_LCG32_DRAW, "draw_reduce"), "N1_lcg64_draw": (W.N1_LCG64_DRAW, "draw_reduce"),
+            "N1_lcg64both_draw": (W.N1_LCG64BOTH_DRAW, "draw_reduce"), "N1_lcg64both_u32": (W.N1_LCG64BOTH, "fill_u32")}
     cfg, call = cfgs[workload]
     n = cfg.n_per_stream
     # calibrate on a small slice of the streams, then time one slice of about target_s

@@ -93,7 +93,13 @@ enum {
      * and cannot overlap.  X_0 = kind 4's instance 0 (SM_seed[0..15], R-D7b).  Update, Weyl
      * term (the same for all instances: footnote 4), output, layout, state
      * access and every entry point are exactly kind 4's. */
-    RNG_XS1024W_SKIP = 7
+    RNG_XS1024W_SKIP = 7,
+    /* kind 0's generator and seeds "using the whole state to produce two 32-bit numbers"
+     * (doubles the nominal rate, lowers the quality): draw 2i = 32 most
+     * significant bits of x_i, draw 2i+1 = its 32 least significant bits, then the state
+     * advances (R-F2).  State access as kind 0 (after an odd number of draws the state is
+     * still x_i; the parity of draws_done says which half comes next). */
+    RNG_LCG64_BOTH = 8
 };
 
 enum {

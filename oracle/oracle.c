@@ -227,12 +227,13 @@ uint32_t orc_lcg32_step(uint32_t x) { return 1664525u * x + 1013904223u; }
 orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local, uint64_t seed)
 {
     if (n_local < 1 || first + n_local > n_total || first + n_local < first) return NULL;
-    if (kind < ORC_LCG64 || kind > ORC_XS1024W_SKIP) return NULL;
+    if (kind < ORC_LCG64 || kind > ORC_LCG64_BOTH) return NULL;
     if ((kind == ORC_XS1024W || kind == ORC_XS1024W_SKIP) && (first % 32 || n_local % 32)) return NULL;
     orc_rng *r = (orc_rng *)calloc(1, sizeof *r);
     if (!r) return NULL;
     r->kind = kind; r->n_total = n_total; r->first = first; r->n_local = n_local; r->seed = seed;
     switch (kind) {
+    case ORC_LCG64_BOTH: /* same generator and seeds; only the output rule differs */
     case ORC_LCG64: /* random seeding: x_0^(s) = SM_seed[s] */
         r->lcg = (uint64_t *)malloc(n_local * sizeof(uint64_t));
         for (uint64_t s = 0; s < n_local; s++) r->lcg[s] = orc_splitmix64(seed, first + s);
@@ -346,6 +347,26 @@ void orc_fill_u32(orc_rng *r, uint32_t *out, uint64_t n)
             r->lcg[s] = x;
         }
         break;
+    case ORC_LCG64_BOTH:
+        /* "on using the whole state to produce two 32-bit numbers, the nominal
+         * performance would double (but ... the quality ... would be reduced)".  R-F2: a state x_i
+         * yields draw 2i = its 32 most significant bits, draw 2i+1 = its 32 least significant bits;
+         * the state advances after the second one.  draws_done is common to all streams, so its
+         * parity says which half comes next. */
+#pragma omp parallel for schedule(static)
+        for (uint64_t s = 0; s < S; s++) {
+            uint64_t x = r->lcg[s];
+            for (uint64_t j = 0; j < n; j++) {
+                if (((r->draws_done + j) & 1) == 0) {
+                    out[s * n + j] = (uint32_t)(x >> 32);
+                } else {
+                    out[s * n + j] = (uint32_t)x;
+                    x = orc_lcg64_step(x);
+                }
+            }
+            r->lcg[s] = x;
+        }
+        break;
     case ORC_LCG64_LEAPFROG: {
         /* "all threads generate numbers out of the same global
          * sequence (1)": element m of the global sequence is draw floor(m/S)
@@ -436,7 +457,7 @@ void orc_draw_reduce(orc_rng *r, uint32_t *out, uint64_t n)
 uint64_t orc_state_words32(const orc_rng *r)
 {
     switch (r->kind) {
-    case ORC_LCG64: case ORC_LCG64_LEAPFROG: return 2 * r->n_local;
+    case ORC_LCG64: case ORC_LCG64_BOTH: case ORC_LCG64_LEAPFROG: return 2 * r->n_local;
     case ORC_XORWOW: return 6 * r->n_local;
     case ORC_XS1024W: case ORC_XS1024W_SKIP: return r->n_local;
     case ORC_LCG32: return r->n_local;
@@ -447,7 +468,7 @@ uint64_t orc_state_words32(const orc_rng *r)
 void orc_get_state(const orc_rng *r, uint32_t *out)
 {
     switch (r->kind) {
-    case ORC_LCG64: memcpy(out, r->lcg, r->n_local * 8); break;
+    case ORC_LCG64: case ORC_LCG64_BOTH: memcpy(out, r->lcg, r->n_local * 8); break;
     case ORC_LCG64_LEAPFROG: {
         uint64_t X = r->leap_X; /* X_{t S}; stream s sits at X_{t S + s} */
         for (uint64_t m = 0; m < r->first + r->n_local; m++) {

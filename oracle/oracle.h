@@ -36,8 +36,10 @@ enum {
     ORC_PHILOX4X32_7   = 5, /* the 7-round variant          */
     ORC_LCG32          = 6, /* PAPER.md:33 eq.(1), :46: a=1664525, c=1013904223,
                                m=2^32; draw j = x_j (all 32 bits), x_0 = lo32(SM_seed[s]) */
-    ORC_XS1024W_SKIP   = 7  /* kind 4 seeded as PAPER.md:228 does: all instances from one
+    ORC_XS1024W_SKIP   = 7, /* kind 4 seeded as PAPER.md:228 does: all instances from one
                                state, instance g skipped ahead by g * 2^137 updates     */
+    ORC_LCG64_BOTH     = 8  /* LCG64 "using the whole state to produce two
+                               32-bit numbers": draw 2i = hi32(x_i), draw 2i+1 = lo32(x_i) */
 };
 
 /* ---- elementary pieces, exported so that the tests can pin them ---------- */

@@ -32,6 +32,32 @@ __global__ void __launch_bounds__(256) draw_reduce_kernel(Gen g, uint2 *__restri
         if constexpr (KIND == RNG_XORWOW) sum = add_on_fma_pipe(sum, u, one);
         else sum += u;
     };
+    if constexpr (KIND == RNG_LCG64_BOTH) {
+        // both words of every state: finish a half-used state, then whole states (one
+        // multiply-add per TWO draws, no per-draw parity test), then at most one leading high word
+        uint64_t left = n;
+        if (left && gen.half) {
+            accumulate(gen.next());
+            left--;
+        }
+        uint64_t pairs = left >> 1;
+        uint64_t y = gen.x;
+        while (pairs) {
+            const uint32_t t32 = pairs > 0x40000000ull ? 0x40000000u : (uint32_t)pairs;
+            pairs -= t32;
+#pragma unroll 8
+            for (uint32_t t = 0; t < t32; t++) {
+                accumulate((uint32_t)(y >> 32));
+                accumulate((uint32_t)y);
+                y = kLcgA * y + kLcgC;
+            }
+        }
+        gen.x = y;
+        if (left & 1ull) accumulate(gen.next());
+        gen.store(g, s);
+        out[s] = make_uint2(x, sum);
+        return;
+    }
     uint64_t trips = n / UNROLL;
     const uint32_t rest = (uint32_t)(n - trips * UNROLL);
     while (trips) { // 32-bit inner counter: the 64-bit one costs three uniform instructions per trip
@@ -157,6 +183,7 @@ cudaError_t launch_draw_reduce(const rng_handle &h, uint32_t *d_out, uint64_t n,
     case RNG_PHILOX4X32_10: philox_draw_reduce_kernel<10><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     case RNG_PHILOX4X32_7: philox_draw_reduce_kernel<7><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     case RNG_LCG32: draw_reduce_kernel<RNG_LCG32><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_LCG64_BOTH: draw_reduce_kernel<RNG_LCG64_BOTH><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     default: return cudaErrorInvalidValue;
     }
     count_launch();

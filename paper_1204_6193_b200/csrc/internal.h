@@ -63,6 +63,7 @@ struct rng_handle {
     case RNG_XS1024W: MACRO(RNG_XS1024W); break;                    \
     case RNG_PHILOX4X32_7: MACRO(RNG_PHILOX4X32_7); break;          \
     case RNG_LCG32: MACRO(RNG_LCG32); break;                        \
+    case RNG_LCG64_BOTH: MACRO(RNG_LCG64_BOTH); break;              \
     default: return cudaErrorInvalidValue;                          \
     }
 

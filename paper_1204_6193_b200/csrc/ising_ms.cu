@@ -445,6 +445,7 @@ cudaError_t launch_ising_ms_half_sweep(const rng_handle &h, uint32_t *planes, ui
         case RNG_PHILOX4X32_10: launch_ms_word<RNG_PHILOX4X32_10>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         case RNG_PHILOX4X32_7: launch_ms_word<RNG_PHILOX4X32_7>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         case RNG_LCG32: launch_ms_word<RNG_LCG32>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
+        case RNG_LCG64_BOTH: launch_ms_word<RNG_LCG64_BOTH>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         default: return cudaErrorInvalidValue;
         }
     }

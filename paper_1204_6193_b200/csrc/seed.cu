@@ -102,6 +102,10 @@ cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st)
         seed_lcg64_kernel<<<grid, B, 0, st>>>((uint64_t *)g.state, g.S, g.first, g.seed);
         count_launch(2);
         break;
+    case RNG_LCG64_BOTH: // same seeds as RNG_LCG64; no table (its only kernels step with the plain constants)
+        seed_lcg64_kernel<<<grid, B, 0, st>>>((uint64_t *)g.state, g.S, g.first, g.seed);
+        count_launch();
+        break;
     case RNG_LCG64_LEAPFROG:
         lcg_table_kernel<<<1, 256, 0, st>>>(tab, g.n_total);
         seed_lcg64_leapfrog_kernel<<<grid, B, 0, st>>>((uint64_t *)g.state, g.S, g.first, g.seed);

@@ -34,6 +34,26 @@ template <>
 struct Stream<RNG_LCG64_LEAPFROG> : StreamLcg {
 };
 
+// ---- LCG64, both halves of the state as output (R-F2): high word, low word, advance ----
+template <>
+struct Stream<RNG_LCG64_BOTH> {
+    uint64_t x;
+    uint32_t half; // 0: the high word of x comes next, 1: the low word
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s)
+    {
+        x = ((const uint64_t *)g.state)[s];
+        half = (uint32_t)g.draws_done & 1u; // all streams advance in lockstep
+    }
+    __device__ __forceinline__ uint32_t next()
+    {
+        const uint32_t r = half ? (uint32_t)x : (uint32_t)(x >> 32);
+        if (half) x = kLcgA * x + kLcgC; // eq.(1)
+        half ^= 1u;
+        return r;
+    }
+    __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint64_t *)g.state)[s] = x; }
+};
+
 // ---- XORWOW: six words, interleaved w[k*S + s] ----
 template <>
 struct Stream<RNG_XORWOW> {

@@ -9,7 +9,7 @@ from __future__ import annotations
 
 from dataclasses import dataclass
 
-LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP = range(8)
+LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP, LCG64_BOTH = range(9)
 MASTER_SEED = 1                    # "seeded via splitmix64(master seed 1)" (config 1)
 LATTICE_SEED = 2                   # ising_init_random seed
 BETA_C = 0.44068679350977147       # ln(1+sqrt 2)/2 as a double (config 5)
@@ -63,6 +63,8 @@ N1_PHILOX7_DRAW = FillCfg("N1_philox7_2^22x256", PHILOX4X32_7, 1 << 22, 256)
 N1_PHILOX10_DRAW = FillCfg("N1_philox10_2^22x256", PHILOX4X32_10, 1 << 22, 256)
 N1_LCG32_DRAW = FillCfg("N1_lcg32_2^22x256", LCG32, 1 << 22, 256)
 N1_LCG64_DRAW = FillCfg("N1_lcg64_2^22x256", LCG64, 1 << 22, 256)
+N1_LCG64BOTH_DRAW = FillCfg("N1_lcg64both_2^22x256", LCG64_BOTH, 1 << 22, 256)
+N1_LCG64BOTH = FillCfg("N1_lcg64both_2^20x1024", LCG64_BOTH, 1 << 20, 1024)
 
 # C5a: L=4, beta=0.3 vs exact enumeration; 8 streams (K = 1 site per stream per colour)
 C5A_PHILOX = IsingCfg("C5a_ising_L4_philox", PHILOX4X32_10, 4, 0.3, 8, 1000)

@@ -64,6 +64,7 @@ def test_state_bytes(L):
     assert pkg.rng_state_bytes(pkg.RNG_PHILOX4X32_7, 1 << 20) == 0
     assert pkg.rng_state_bytes(pkg.RNG_LCG32, 1000) == 4000            # "32 bits" PAPER.md:262 (Table 2)
     assert pkg.rng_state_bytes(pkg.RNG_XS1024W_SKIP, 64) == 256
+    assert pkg.rng_state_bytes(pkg.RNG_LCG64_BOTH, 3) == 24
     assert pkg.rng_state_bytes(99, 5) == 0
 
 

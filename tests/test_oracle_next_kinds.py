@@ -72,3 +72,30 @@ def test_uniformity_of_the_extra_kinds():
         assert abs(f.var() - 1 / 12) < 3 * np.sqrt(1 / (180 * n))
         chi2 = ((np.bincount((f * 256).astype(int), minlength=256) - n / 256) ** 2 / (n / 256)).sum()
         assert 187 < chi2 < 323, (kind, chi2)
+
+
+def test_lcg64_both_words_is_the_64_bit_sequence_cut_in_two():
+    # the whole 64-bit state as two 32-bit numbers.  Against the big-integer recurrence
+    # of eq.(1) with the constants of PAPER.md:46, high word first (R-F2); any split of
+    # the calls, odd ones included, continues the same stream; the plain LCG64 kind is its even draws.
+    a, c, m = 2862933555777941757, 1442695040888963407, 1 << 64
+    S, seed, n = 3, 21, 11
+    out = oracle.Rng(8, S, seed).fill_u32(n).reshape(S, n)
+    for s in range(S):
+        x = oracle.splitmix64(seed, s)
+        want = []
+        while len(want) < n:
+            want += [x >> 32, x & 0xFFFFFFFF]
+            x = (a * x + c) % m
+        assert [int(v) for v in out[s]] == want[:n]
+    r = oracle.Rng(8, S, seed)
+    parts = [r.fill_u32(k).reshape(S, k) for k in (1, 3, 2, 5)]
+    assert np.array_equal(np.concatenate(parts, axis=1), out)
+    assert np.array_equal(oracle.Rng(oracle.LCG64, S, seed).fill_u32(5).reshape(S, 5), out[:, 0:10:2])
+    # state after an odd number of draws is still x_i (it advances after the low word)
+    r = oracle.Rng(8, S, seed)
+    r.fill_u32(1)
+    st = r.get_state().view(np.uint64)
+    assert [int(v) for v in st] == [oracle.splitmix64(seed, s) for s in range(S)]
+    r.fill_u32(1)
+    assert [int(v) for v in r.get_state().view(np.uint64)] == [(a * oracle.splitmix64(seed, s) + c) % m for s in range(S)]

@@ -30,7 +30,7 @@ def _worker(rank: int, world: int, port: int, n_per_rank: int, n: int):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         for kind in (W.LCG64, W.LCG64_LEAPFROG, W.XORWOW, W.PHILOX4X32_10, W.XS1024W, W.PHILOX4X32_7, W.LCG32,
-                     W.XS1024W_SKIP):
+                     W.XS1024W_SKIP, W.LCG64_BOTH):
             # bench.py's weak-scaling layout
             n_total, first, n_local = sharding.weak_scaling_shard(rank, world, n_per_rank)
             mine = oracle.Rng(kind, n_local, W.MASTER_SEED, first=first, n_total=n_total).fill_u32(n)
