@@ -219,7 +219,40 @@ struct orc_rng {
     uint32_t *xw;         /* XORWOW: [n_local][6] */
     uint32_t *xs;         /* XS1024W: [n_local/32][32], word i of instance g at 32 g + i */
     uint32_t *lcg32;      /* LCG32: x of each local stream */
+    float *lf;            /* LFIB: [n_local/256][r], the last r numbers of each instance, oldest first */
 };
+
+/* ---- lagged Fibonacci, PAPER.md:105-124 ---------------------------------------------
+ * eq.(5):  u_n = u_{n-r} + u_{n-s} (mod 1)  "by using floating-point arithmetic",
+ * with (r,s) = (521,353) and (1279,861).  Single precision:  t = a + b; if
+ * (t >= 1) t -= 1.  R-G1: the seeds are 23-bit fractions, so that every sum is exact in
+ * float (a sum in [1,2) has spacing 2^-23) and the float recurrence IS addition mod 1.
+ * The ring buffer is shared by the threads of a block, which produce s numbers at a
+ * time: R-G2: an INSTANCE serves T = 256 streams (threads), T <= s; the
+ * instance's numbers v_0, v_1, ... (v_m = u_{r+m}) are dealt round-robin: stream t of
+ * the instance gets v_{jT+t} as its draw j.  R-G3: u_i of instance g, i < r, is
+ * (w >> 9) 2^-23 with w the 32-bit word number g r + i of the splitmix64 word sequence
+ * (word 2k = lo32, 2k+1 = hi32 of SM_seed[k]); if no u_i of an instance is an odd
+ * multiple of 2^-23 its u_0 gets that bit (an all-even seed would halve the period [19]).
+ * As 32-bit integers the draws are (v 2^23) << 9, so that the fixed map gives v back. */
+#define ORC_LFIB_T 256
+static int lfib_lags(int kind, int *r, int *s)
+{
+    if (kind == ORC_LFIB521) { *r = 521; *s = 353; return 1; }
+    if (kind == ORC_LFIB1279) { *r = 1279; *s = 861; return 1; }
+    return 0;
+}
+float orc_lfib_add(float a, float b)
+{
+    volatile float t = a + b; /* one IEEE single-precision addition, no wider intermediate */
+    if (t >= 1.0f) t = t - 1.0f;
+    return t;
+}
+static uint32_t splitmix_word32(uint64_t seed, uint64_t w)
+{
+    uint64_t z = orc_splitmix64(seed, w / 2);
+    return (w & 1) ? (uint32_t)(z >> 32) : (uint32_t)z;
+}
 
 /* G1: 32-bit LCG, eq.(1) with the constants of PAPER.md:46 */
 uint32_t orc_lcg32_step(uint32_t x) { return 1664525u * x + 1013904223u; }
@@ -227,7 +260,8 @@ uint32_t orc_lcg32_step(uint32_t x) { return 1664525u * x + 1013904223u; }
 orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local, uint64_t seed)
 {
     if (n_local < 1 || first + n_local > n_total || first + n_local < first) return NULL;
-    if (kind < ORC_LCG64 || kind > ORC_LCG64_BOTH) return NULL;
+    if (kind < ORC_LCG64 || kind > ORC_LFIB1279) return NULL;
+    if ((kind == ORC_LFIB521 || kind == ORC_LFIB1279) && (first % ORC_LFIB_T || n_local % ORC_LFIB_T)) return NULL;
     if ((kind == ORC_XS1024W || kind == ORC_XS1024W_SKIP) && (first % 32 || n_local % 32)) return NULL;
     orc_rng *r = (orc_rng *)calloc(1, sizeof *r);
     if (!r) return NULL;
@@ -274,6 +308,24 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
             if (!any) X[31] = 1;
         }
         break;
+    case ORC_LFIB521:
+    case ORC_LFIB1279: { /* random seeding of the ring buffers, PAPER.md:122 ("it appears safe to just seed") */
+        int lr, ls;
+        lfib_lags(kind, &lr, &ls);
+        r->lf = (float *)malloc(n_local / ORC_LFIB_T * (uint64_t)lr * sizeof(float));
+        for (uint64_t g = 0; g < n_local / ORC_LFIB_T; g++) {
+            uint64_t gg = first / ORC_LFIB_T + g;
+            float *h = r->lf + g * (uint64_t)lr;
+            int odd = 0;
+            for (int i = 0; i < lr; i++) {
+                uint32_t k = splitmix_word32(seed, gg * (uint64_t)lr + (uint64_t)i) >> 9;
+                odd |= (int)(k & 1u);
+                h[i] = (float)k * 0x1p-23f;
+            }
+            if (!odd) h[0] += 0x1p-23f; /* k even, so k+1 < 2^23: still a 23-bit fraction */
+        }
+        break;
+    }
     case ORC_XS1024W_SKIP: {
         /* every instance starts from the SAME state and skips g * 2^137 updates,
          * g = global instance number, by multiplying with J = M^(2^137) once per instance.
@@ -304,7 +356,7 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
 void orc_destroy(orc_rng *r)
 {
     if (!r) return;
-    free(r->lcg); free(r->xw); free(r->xs); free(r->lcg32); free(r);
+    free(r->lcg); free(r->xw); free(r->xs); free(r->lcg32); free(r->lf); free(r);
 }
 
 uint64_t orc_draws_done(const orc_rng *r) { return r->draws_done; }
@@ -406,6 +458,27 @@ void orc_fill_u32(orc_rng *r, uint32_t *out, uint64_t n)
             r->lcg32[s] = x;
         }
         break;
+    case ORC_LFIB521:
+    case ORC_LFIB1279: {
+        int lr, ls;
+        lfib_lags(r->kind, &lr, &ls);
+#pragma omp parallel for schedule(static)
+        for (uint64_t g = 0; g < S / ORC_LFIB_T; g++) {
+            /* the instance's sequence, one number after the other: hist = u_{n-r} .. u_{n-1} */
+            float *hist = r->lf + g * (uint64_t)lr;
+            float *u = (float *)malloc(((uint64_t)lr + n * ORC_LFIB_T) * sizeof(float));
+            memcpy(u, hist, (size_t)lr * sizeof(float));
+            for (uint64_t m = 0; m < n * ORC_LFIB_T; m++) {
+                uint64_t i = (uint64_t)lr + m;                 /* u[i] = u[i-r] + u[i-s] mod 1, eq.(5) */
+                u[i] = orc_lfib_add(u[i - (uint64_t)lr], u[i - (uint64_t)ls]);
+                /* v_m is draw m / T of stream m % T of this instance (R-G2) */
+                out[(g * ORC_LFIB_T + m % ORC_LFIB_T) * n + m / ORC_LFIB_T] = (uint32_t)(u[i] * 0x1p23f) << 9;
+            }
+            memcpy(hist, u + n * ORC_LFIB_T, (size_t)lr * sizeof(float));
+            free(u);
+        }
+        break;
+    }
     case ORC_XS1024W:
     case ORC_XS1024W_SKIP:
         /* stream s = word (s mod 32) of instance floor(s/32)  (R-D4) */
@@ -461,6 +534,8 @@ uint64_t orc_state_words32(const orc_rng *r)
     case ORC_XORWOW: return 6 * r->n_local;
     case ORC_XS1024W: case ORC_XS1024W_SKIP: return r->n_local;
     case ORC_LCG32: return r->n_local;
+    case ORC_LFIB521: return r->n_local / ORC_LFIB_T * 521;
+    case ORC_LFIB1279: return r->n_local / ORC_LFIB_T * 1279;
     default: return 0;
     }
 }
@@ -480,6 +555,7 @@ void orc_get_state(const orc_rng *r, uint32_t *out)
     case ORC_XORWOW: memcpy(out, r->xw, r->n_local * 24); break;
     case ORC_XS1024W: case ORC_XS1024W_SKIP: memcpy(out, r->xs, r->n_local * 4); break;
     case ORC_LCG32: memcpy(out, r->lcg32, r->n_local * 4); break;
+    case ORC_LFIB521: case ORC_LFIB1279: memcpy(out, r->lf, orc_state_words32(r) * 4); break; /* float bit patterns */
     default: break;
     }
 }

@@ -38,8 +38,10 @@ enum {
                                m=2^32; draw j = x_j (all 32 bits), x_0 = lo32(SM_seed[s]) */
     ORC_XS1024W_SKIP   = 7, /* kind 4 seeded as PAPER.md:228 does: all instances from one
                                state, instance g skipped ahead by g * 2^137 updates     */
-    ORC_LCG64_BOTH     = 8  /* LCG64 "using the whole state to produce two
+    ORC_LCG64_BOTH     = 8, /* LCG64 "using the whole state to produce two
                                32-bit numbers": draw 2i = hi32(x_i), draw 2i+1 = lo32(x_i) */
+    ORC_LFIB521        = 9, /* PAPER.md:105-124 eq.(5): u_n = u_{n-r} + u_{n-s} mod 1 in float,   */
+    ORC_LFIB1279       = 10 /* (r,s) = (521,353) / (1279,861); ring shared by 256 streams        */
 };
 
 /* ---- elementary pieces, exported so that the tests can pin them ---------- */
@@ -74,6 +76,9 @@ void orc_xs1024_vecmat(const uint32_t X[32], const uint32_t *A, uint32_t out[32]
 void orc_xs1024_matmul(const uint32_t *A, const uint32_t *B, uint32_t *out);
 void orc_xs1024_matpow2(unsigned k, uint32_t *out);
 
+/* eq.(5): one float addition mod 1 */
+float orc_lfib_add(float a, float b);
+
 /* fixed output map u32 -> [0,1) float:  (u >> 8) * 2^-24   (BASELINE.json) */
 float orc_u32_to_f32(uint32_t u);
 
@@ -100,7 +105,8 @@ void orc_draw_reduce(orc_rng *, uint32_t *out, uint64_t n);
  *   LCG64 / LEAPFROG: n_local x u64 (x of each stream, LEAPFROG: X_{s + t*S})
  *   XORWOW: n_local x 6 x u32 {x,y,z,w,v,d}, stream-major
  *   PHILOX: nothing (0 words)
- *   XS1024W: n_local x u32 (word `lane` of instance s/32 at index s)        */
+ *   XS1024W: n_local x u32 (word `lane` of instance s/32 at index s)
+ *   LFIB: per instance (256 streams) the last r numbers, oldest first, as float bits */
 uint64_t orc_state_words32(const orc_rng *);
 void     orc_get_state(const orc_rng *, uint32_t *out);
 
