@@ -99,7 +99,22 @@ enum {
      * significant bits of x_i, draw 2i+1 = its 32 least significant bits, then the state
      * advances (R-F2).  State access as kind 0 (after an odd number of draws the state is
      * still x_i; the parity of draws_done says which half comes next). */
-    RNG_LCG64_BOTH = 8
+    RNG_LCG64_BOTH = 8,
+    /* The paper's second generator with state shared by the threads of a block: the additive
+     * lagged Fibonacci generator on floats, u_n = u_{n-r} + u_{n-s} (mod 1), single precision
+     * (eq.(5)), lags (r,s) = (521,353) and (1279,861).
+     * R-G1..G3: an INSTANCE (one ring buffer) serves 256 consecutive streams (n_streams and
+     * first must be multiples of 256); its numbers v_0, v_1, ... are dealt round-robin, stream
+     * t of the instance gets v_{256 j + t} as draw j.  Seeds: u_i of instance g, i < r, is
+     * (w >> 9) 2^-23 with w the 32-bit word g r + i of the splitmix64 word sequence (word 2k =
+     * lo32, 2k+1 = hi32 of SM_seed[k]); an instance without an odd multiple of 2^-23 gets
+     * that bit on u_0.  All values are 23-bit fractions, every addition is exact.  fill_f32
+     * writes the numbers themselves; as 32-bit integers they are (v 2^23) << 9, so the fixed
+     * map (u >> 8) 2^-24 gives v back.  State: per instance its last r numbers, oldest first,
+     * as float bit patterns.  Plain ising_sweep only (byte kernel); ising_sweep_multihit
+     * returns RNG_E_UNSUPPORTED. */
+    RNG_LFIB521 = 9,
+    RNG_LFIB1279 = 10
 };
 
 enum {

@@ -74,6 +74,8 @@ uint64_t rng_state_bytes(int kind, uint64_t n)
     case RNG_XS1024W:
     case RNG_XS1024W_SKIP:
     case RNG_LCG32: return 4 * n;
+    case RNG_LFIB521: return 4ull * 521ull * (n / 256);
+    case RNG_LFIB1279: return 4ull * 1279ull * (n / 256);
     default: return 0;
     }
 }
@@ -82,12 +84,14 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
 {
     if (!out) return fail(RNG_E_INVAL, "rng_create: out is NULL");
     *out = nullptr;
-    if (kind < RNG_LCG64 || kind > RNG_LCG64_BOTH) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
+    if (kind < RNG_LCG64 || kind > RNG_LFIB1279) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
     if (n_local < 1 || first + n_local < first || first + n_local > n_total)
         return fail(RNG_E_INVAL, "rng_create: stream range [%llu,+%llu) not inside [0,%llu)", (unsigned long long)first,
                     (unsigned long long)n_local, (unsigned long long)n_total);
     if ((kind == RNG_XS1024W || kind == RNG_XS1024W_SKIP) && ((first | n_local) & 31ull))
         return fail(RNG_E_INVAL, "rng_create: RNG_XS1024W needs whole 32-stream instances");
+    if ((kind == RNG_LFIB521 || kind == RNG_LFIB1279) && ((first | n_local) & 255ull))
+        return fail(RNG_E_INVAL, "rng_create: RNG_LFIB* needs whole 256-stream instances");
     if (n_local > (1ull << 38)) return fail(RNG_E_INVAL, "rng_create: too many streams");
     int dev = 0, ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
@@ -115,7 +119,10 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
     if (e == cudaSuccess && (kind == RNG_LCG64 || kind == RNG_LCG64_LEAPFROG)) e = cudaMalloc(&tab, sizeof(LcgTable));
     h->g.lcg = tab;
     if (e == cudaSuccess) e = cudaMalloc(&h->energy_scratch, sizeof(int64_t));
-    if (e == cudaSuccess) e = (kind == RNG_XS1024W_SKIP) ? launch_seed_xs1024_skip(h->g, 0) : launch_seed(h->g, tab, 0);
+    if (e == cudaSuccess)
+        e = (kind == RNG_XS1024W_SKIP)                       ? launch_seed_xs1024_skip(h->g, 0)
+            : (kind == RNG_LFIB521 || kind == RNG_LFIB1279) ? launch_seed_lfib(h->g, 0)
+                                                            : launch_seed(h->g, tab, 0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(0);
     if (e != cudaSuccess) {
         int rc = cuda_fail(e, "rng_create");
@@ -254,6 +261,8 @@ int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta
         return fail(RNG_E_INVAL, "ising_sweep_multihit: tile must be even, 2..44, divide L, with L/tile even");
     if (k_hits < 1) return fail(RNG_E_INVAL, "ising_sweep_multihit: k_hits must be >= 1");
     if (h->g.S != (uint64_t)L * L / 4) return fail(RNG_E_INVAL, "ising_sweep_multihit: needs n_streams == L*L/4");
+    if (h->g.kind == RNG_LFIB521 || h->g.kind == RNG_LFIB1279)
+        return fail(RNG_E_UNSUPPORTED, "ising_sweep_multihit: RNG_LFIB* shares its state across a 256-thread CTA; use ising_sweep");
     if (h->g.kind == RNG_XS1024W && (tile * tile / 2u) % 32u)
         return fail(RNG_E_INVAL, "ising_sweep_multihit: this kind needs whole warps per tile (tile a multiple of 8)");
     const uint64_t per_sweep = 4ull * k_hits;

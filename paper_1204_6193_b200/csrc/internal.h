@@ -24,6 +24,7 @@ struct LcgTable {
 //   PHILOX           : none
 //   XS1024W          : u32 w[S]      (word `lane` of instance g at w[32 g + lane])
 //   LCG32            : u32 x[S]
+//   LFIB521 / 1279   : float u[S/256][r]  (an instance's last r numbers, oldest first)
 struct Gen {
     int kind;
     uint64_t S;          // local streams
@@ -73,6 +74,9 @@ void count_launch(uint64_t n = 1);
 
 // seed.cu
 cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st);
+// lfib.cu (RNG_LFIB521 / RNG_LFIB1279: seeding and fill; draws and Ising go through Stream<KIND>)
+cudaError_t launch_seed_lfib(const Gen &g, cudaStream_t st);
+cudaError_t launch_lfib_fill(const Gen &g, void *d_out, uint64_t n, bool f32, cudaStream_t st);
 // seed_xs1024_skip.cu (RNG_XS1024W_SKIP; synchronises the stream, frees its scratch)
 cudaError_t launch_seed_xs1024_skip(const Gen &g, cudaStream_t st);
 // fill.cu  (f32 = apply the (u>>8)*2^-24 map; out is uint32_t* or float*)

@@ -230,6 +230,7 @@ cudaError_t launch_ising_half_sweep(const rng_handle &h, int8_t *d_spins, uint32
         const bool geom_ok = (L % 16u) == 0u && L >= 16u && L <= 65536u && h.var_ising != 1;
         bool kind_ok;
         if (kind_is_philox(g.kind)) kind_ok = (K % 4ull) == 0ull && (draws_done % 4ull) == 0ull;
+        else if (kind_is_lfib(g.kind)) kind_ok = false; // CTA-shared state: the generic kernel's thread <-> stream map only
         else if (g.kind == RNG_XS1024W) kind_ok = K == 8ull && (cpr % 32u) == 0u;
         else kind_ok = K == 8ull;
         if (thr_ok && geom_ok && kind_ok) {
@@ -250,7 +251,11 @@ cudaError_t launch_ising_half_sweep(const rng_handle &h, int8_t *d_spins, uint32
     if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
 #define GENERIC(KIND) \
     ising_half_sweep_generic_kernel<KIND><<<(unsigned)grid, 256, 0, st>>>(g, d_spins, L, tab, K, colour)
-    RNGB200_DISPATCH_KIND(g.kind, GENERIC)
+    if (g.kind == RNG_LFIB521) GENERIC(RNG_LFIB521);
+    else if (g.kind == RNG_LFIB1279) GENERIC(RNG_LFIB1279);
+    else {
+        RNGB200_DISPATCH_KIND(g.kind, GENERIC)
+    }
 #undef GENERIC
     count_launch();
     return cudaGetLastError();

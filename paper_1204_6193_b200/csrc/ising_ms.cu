@@ -370,6 +370,7 @@ __global__ void __launch_bounds__(256) ising_ms_energy_kernel(const uint32_t *__
 bool ising_ms_eligible(const rng_handle &h, uint32_t L, const IsingTable &tab, uint64_t K, uint64_t draws_done)
 {
     if (L % 64u || L > 65536u) return false;
+    if (h.g.kind == RNG_LFIB521 || h.g.kind == RNG_LFIB1279) return false; // CTA-shared state: byte kernel only
     const uint32_t one = 1u << 24;
     if (tab.T[0] != one || tab.T[1] != one || tab.T[2] != one) return false;
     if (tab.T[4] < 1u || tab.T[4] > tab.T[3] || tab.T[3] > one) return false;

@@ -4,6 +4,7 @@
 // Product code (sm_100a); shares nothing with oracle/.
 #pragma once
 #include "internal.h"
+#include "lfib.cuh"
 
 namespace rngb200 {
 
@@ -128,6 +129,14 @@ struct Stream<RNG_PHILOX4X32_10> : StreamPhilox<10> {
 };
 template <>
 struct Stream<RNG_PHILOX4X32_7> : StreamPhilox<7> {
+};
+
+// ---- float lagged Fibonacci, ring shared by the 256 threads of the CTA (lfib.cuh) ----
+template <>
+struct Stream<RNG_LFIB521> : LfibStream<RNG_LFIB521> {
+};
+template <>
+struct Stream<RNG_LFIB1279> : LfibStream<RNG_LFIB1279> {
 };
 
 // ---- XORShift1024/Weyl, cooperative: lane = word index; whole warps only ----

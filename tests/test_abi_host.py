@@ -65,6 +65,8 @@ def test_state_bytes(L):
     assert pkg.rng_state_bytes(pkg.RNG_LCG32, 1000) == 4000            # "32 bits" PAPER.md:262 (Table 2)
     assert pkg.rng_state_bytes(pkg.RNG_XS1024W_SKIP, 64) == 256
     assert pkg.rng_state_bytes(pkg.RNG_LCG64_BOTH, 3) == 24
+    assert pkg.rng_state_bytes(pkg.RNG_LFIB521, 512) == 2 * 521 * 4    # one ring of r words per 256 streams
+    assert pkg.rng_state_bytes(pkg.RNG_LFIB1279, 256) == 1279 * 4
     assert pkg.rng_state_bytes(99, 5) == 0
 
 

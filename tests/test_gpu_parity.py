@@ -15,6 +15,7 @@ import paper_1204_6193_b200 as pkg  # noqa: E402
 KINDS = list(pkg.KIND_NAMES)
 IDS = [pkg.KIND_NAMES[k] for k in KINDS]
 XS_KINDS = (pkg.RNG_XS1024W, pkg.RNG_XS1024W_SKIP)
+LFIB_KINDS = (pkg.RNG_LFIB521, pkg.RNG_LFIB1279)  # one ring buffer per 256 streams
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -37,6 +38,8 @@ def host(t, n, dtype=np.uint32):
 
 
 def n_streams_for(kind, S):
+    if kind in LFIB_KINDS:
+        return max(256, S - S % 256)
     return S - S % 32 if kind in XS_KINDS else S
 
 
@@ -107,6 +110,7 @@ def test_mixed_call_sequence_is_one_stream(kind):
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 @pytest.mark.parametrize("S,ns", [(2048 + 96, (256, 1, 0, 3, 1001)), (32, (5,))])
 def test_draw_reduce(kind, S, ns):
+    S = n_streams_for(kind, S)
     g, o = pkg.Rng(kind, S, 7), oracle.Rng(kind, S, 7)
     for n in ns:
         out = dev_u32(2 * S)
@@ -171,7 +175,7 @@ def test_xs1024_lane_layouts_are_one_generator(K, store):
 # ---------------------------------------------------------------------------------
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 def test_shard_equals_rows_of_the_whole(kind):
-    n_total, first, n_local, n = 640, 256, 160, 20
+    n_total, first, n_local, n = (1280, 256, 512, 20) if kind in LFIB_KINDS else (640, 256, 160, 20)
     whole = oracle.Rng(kind, n_total, 3).fill_u32(n).reshape(n_total, n)
     g = pkg.Rng(kind, n_local, 3, first=first, n_total=n_total)
     if g.state_bytes():
@@ -265,7 +269,7 @@ def test_ising_init_and_energy():
                                         (128, 32, 4), (256, 4096, 5), (512, 16384, 3), (48, 96, 5), (64, 512, 4),
                                         (1024, 1024, 2)])
 def test_ising_sweep_bit_exact(kind, L, S, sweeps):
-    if kind in XS_KINDS and S % 32:
+    if (kind in XS_KINDS and S % 32) or (kind in LFIB_KINDS and S % 256):
         pytest.skip("xs1024 needs whole 32-stream instances")
     beta = 0.3 if L == 4 else 0.44068679350977147
     g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
@@ -294,7 +298,7 @@ def test_ising_sweep_bit_exact(kind, L, S, sweeps):
 def test_ising_kernel_variants_share_one_trajectory(kind, L, S, sweeps, variant):
     """every kernel variant (generic byte kernel, 16-byte chunk kernel, multi-spin bit planes in
     STREAM and WORD mode) reproduces the oracle's lattice, energy trace and generator state"""
-    if kind in XS_KINDS and S % 32:
+    if (kind in XS_KINDS and S % 32) or (kind in LFIB_KINDS and S % 256):
         pytest.skip("xs1024 needs whole 32-stream instances")
     beta = 0.44068679350977147
     g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
@@ -394,7 +398,7 @@ def test_host_entry_points(kind):
     g.draw_reduce_host(r, 33)
     assert np.array_equal(r, o.draw_reduce(33))
     g.close()
-    L, S = 64, 128
+    L, S = 64, (256 if kind in LFIB_KINDS else 128)
     g, o = pkg.Rng(kind, S, 1), oracle.Rng(kind, S, 1)
     sp = oracle.ising_init_random(L, 2)
     ref = sp.copy()
@@ -528,6 +532,8 @@ def test_ising_multihit_bit_exact(kind, L, T, k, sweeps):
     S = L * L // 4
     if kind in XS_KINDS and (S % 32 or (T * T // 2) % 32):
         pytest.skip("whole warp instances per tile only")
+    if kind in LFIB_KINDS:
+        pytest.skip("CTA-shared state: plain ising_sweep only (RNG_E_UNSUPPORTED is tested below)")
     beta = 0.44068679350977147
     g, o = pkg.Rng(kind, S, 13), oracle.Rng(kind, S, 13)
     sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
@@ -558,6 +564,12 @@ def test_ising_multihit_argument_errors():
     with pytest.raises(pkg.RngError):
         g.ising_sweep_multihit(sp, 8, 0.3, 1, 2, 1)
     g.close()
+    g = pkg.Rng(pkg.RNG_LFIB521, 256, 1)               # CTA-shared state does not fit the tile <-> CTA map
+    sp = torch.ones(32 * 32, dtype=torch.int8, device="cuda")
+    with pytest.raises(pkg.RngError) as e:
+        g.ising_sweep_multihit(sp, 32, 0.3, 1, 8, 1)
+    assert e.value.code == pkg.RNG_E_UNSUPPORTED
+    g.close()
 
 
 @pytest.mark.parametrize("kind", [pkg.RNG_PHILOX4X32_10, pkg.RNG_XORWOW, pkg.RNG_XS1024W_SKIP],
@@ -579,4 +591,43 @@ def test_table1_multihit_L1024_beta04_energy_within_3_sigma(kind):
     bins = e.reshape(-1, 500).mean(axis=1)
     sigma = bins.std(ddof=1) / np.sqrt(len(bins))
     assert abs(e.mean() - ex["e"]) < 3 * sigma, (e.mean(), ex["e"], sigma)
+    g.close()
+
+
+@pytest.mark.parametrize("kind", LFIB_KINDS, ids=["r521", "r1279"])
+def test_lfib_ring_wraps_many_times_and_state_round_trips(kind):
+    """long runs (the 1024 / 2048-word ring wraps hundreds of times), ragged n, f32 = the numbers themselves,
+    checkpoint / resume through get_state / set_state, Ising on the byte kernel with K = 32 draws per stream"""
+    S = 3 * 256
+    g, o = pkg.Rng(kind, S, 17), oracle.Rng(kind, S, 17)
+    for n in (1000, 1, 31, 33, 0, 64):
+        out = dev_u32(S * n)
+        g.fill_u32(out, n)
+        assert np.array_equal(host(out, S * n), o.fill_u32(n)), n
+    f = torch.empty(S * 77, dtype=torch.float32, device="cuda")
+    g.fill_f32(f, 77)
+    fo = o.fill_f32(77)
+    assert np.array_equal(f.cpu().numpy().view(np.uint32), fo.view(np.uint32))
+    assert fo.min() >= 0.0 and fo.max() < 1.0
+    st = g.get_state()
+    assert np.array_equal(st, o.get_state())
+    red = dev_u32(2 * S)
+    g.draw_reduce(red, 5000)
+    want = o.draw_reduce(5000)
+    assert np.array_equal(host(red, 2 * S), want)
+    g2 = pkg.Rng(kind, S, 999)                      # another seed, then restored from the checkpoint
+    g2.set_state(st)
+    g2.draw_reduce(red, 5000)
+    assert np.array_equal(host(red, 2 * S), want)
+    g2.close()
+    L = 256                                          # K = L*L/2/S = 128/3 not integral -> use S = 1024
+    g.close()
+    g, o = pkg.Rng(kind, 1024, 3), oracle.Rng(kind, 1024, 3)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, 6)
+    sp_o = oracle.ising_init_random(L, 6)
+    tr = torch.empty(6, dtype=torch.int64, device="cuda")
+    g.ising_sweep(sp, L, 0.4, 6, tr)
+    tr_o = o.ising_sweep(sp_o, L, 0.4, 6, trace=True)
+    assert np.array_equal(sp.cpu().numpy(), sp_o) and np.array_equal(tr.cpu().numpy(), tr_o)
     g.close()
