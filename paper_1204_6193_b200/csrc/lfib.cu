@@ -40,11 +40,25 @@ __global__ void __launch_bounds__(LFIB_T) lfib_fill_kernel(Gen g, uint32_t *__re
     const uint32_t t = threadIdx.x, lane = t & 31u, warp = t >> 5;
     LfibStream<KIND> gen;
     gen.load(g, s0 + t);
+    constexpr int NB = LfibStream<KIND>::NB;
+    typename LfibStream<KIND>::Group gr;
+    gen.group_init(gr);
     for (uint64_t j0 = 0; j0 < n; j0 += 32) {
         const uint32_t kk = (uint32_t)((n - j0 < 32ull) ? (n - j0) : 32ull);
-        for (uint32_t q = 0; q < kk; q++) {
-            const float v = gen.next_float();
-            tile[t * 33u + q] = F32 ? __float_as_uint(v) : lfib_u32(v);
+        if (kk == 32u) { // whole groups of NB batches: constant ring addresses (NB divides 32)
+#pragma unroll 1
+            for (uint32_t q0 = 0; q0 < 32u; q0 += NB) {
+#pragma unroll
+                for (int q = 0; q < NB; q++) {
+                    const float v = gen.group_step(gr, q);
+                    tile[t * 33u + q0 + q] = F32 ? __float_as_uint(v) : lfib_u32(v);
+                }
+            }
+        } else {
+            for (uint32_t q = 0; q < kk; q++) { // ragged last tile of the call
+                const float v = gen.next_float();
+                tile[t * 33u + q] = F32 ? __float_as_uint(v) : lfib_u32(v);
+            }
         }
         // next_float() ended with a barrier: the tile is complete
         for (uint32_t r = 0; r < 32u; r++) {
@@ -54,6 +68,51 @@ __global__ void __launch_bounds__(LFIB_T) lfib_fill_kernel(Gen g, uint32_t *__re
         __syncthreads(); // before the tile is overwritten
     }
     gen.store(g, s0 + t);
+}
+
+// In-register draw mode: {xor, sum} of the n draws of every stream; whole groups first, then the rest.
+template <int KIND>
+__global__ void __launch_bounds__(LFIB_T) lfib_draw_kernel(Gen g, uint2 *__restrict__ out, uint64_t n)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * LFIB_T + threadIdx.x;
+    LfibStream<KIND> gen;
+    gen.load(g, s);
+    constexpr int NB = LfibStream<KIND>::NB;
+    typename LfibStream<KIND>::Group gr;
+    gen.group_init(gr);
+    uint32_t x = 0u, sum = 0u;
+    uint64_t groups = n / NB;
+    const uint32_t rest = (uint32_t)(n - groups * NB);
+    while (groups) {
+        const uint32_t g32 = groups > 0x40000000ull ? 0x40000000u : (uint32_t)groups;
+        groups -= g32;
+#pragma unroll 1
+        for (uint32_t i = 0; i < g32; i++) {
+#pragma unroll
+            for (int q = 0; q < NB; q++) {
+                const uint32_t u = lfib_u32(gen.group_step(gr, q));
+                x ^= u;
+                sum += u;
+            }
+        }
+    }
+    for (uint32_t j = 0; j < rest; j++) {
+        const uint32_t u = gen.next();
+        x ^= u;
+        sum += u;
+    }
+    gen.store(g, s);
+    out[s] = make_uint2(x, sum);
+}
+
+cudaError_t launch_lfib_draw(const Gen &g, uint32_t *d_out, uint64_t n, cudaStream_t st)
+{
+    const uint64_t inst = g.S / LFIB_T;
+    if (inst > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+    if (g.kind == RNG_LFIB1279) lfib_draw_kernel<RNG_LFIB1279><<<(unsigned)inst, LFIB_T, 0, st>>>(g, (uint2 *)d_out, n);
+    else lfib_draw_kernel<RNG_LFIB521><<<(unsigned)inst, LFIB_T, 0, st>>>(g, (uint2 *)d_out, n);
+    count_launch();
+    return cudaGetLastError();
 }
 
 cudaError_t launch_seed_lfib(const Gen &g, cudaStream_t st)

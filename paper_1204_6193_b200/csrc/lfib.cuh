@@ -27,8 +27,10 @@ __device__ __forceinline__ float lfib_add(float a, float b)
     const float t = __fadd_rn(a, b);
     return t >= 1.0f ? __fsub_rn(t, 1.0f) : t;
 }
-// the draw as a 32-bit integer: (v 2^23) << 9, so that (u >> 8) 2^-24 == v
-__device__ __forceinline__ uint32_t lfib_u32(float v) { return __float2uint_rz(v * 8388608.0f) << 9; }
+// the draw as a 32-bit integer: (v 2^23) << 9, so that (u >> 8) 2^-24 == v.  v is a 23-bit fraction, so
+// 1 + v is exact and its mantissa field IS v 2^23: shifting the bit pattern left by 9 drops sign and
+// exponent (one FADD + one shift instead of a float -> int conversion on the slow conversion unit).
+__device__ __forceinline__ uint32_t lfib_u32(float v) { return __float_as_uint(__fadd_rn(v, 1.0f)) << 9; }
 
 template <int KIND>
 struct LfibStream {
@@ -59,6 +61,33 @@ struct LfibStream {
         return v;
     }
     __device__ __forceinline__ uint32_t next() { return lfib_u32(next_float()); }
+
+    // Batched form for kernels that draw in groups of NB = RB/256 batches: after NB batches the ring index is
+    // back where it started, so the three ring addresses of batch q of a group are per-thread constants.
+    // A group must start with pos == R (true at load() and after any number of whole groups).
+    static constexpr int NB = RB / LFIB_T;
+    struct Group {
+        const float *a[NB], *b[NB];
+        float *w[NB];
+    };
+    __device__ __forceinline__ void group_init(Group &gr) const
+    {
+#pragma unroll
+        for (int q = 0; q < NB; q++) {
+            const uint32_t n = (uint32_t)R + threadIdx.x + (uint32_t)(LFIB_T * q);
+            gr.a[q] = ring + ((n - R) & (RB - 1));
+            gr.b[q] = ring + ((n - S) & (RB - 1));
+            gr.w[q] = ring + (n & (RB - 1));
+        }
+    }
+    // batch q of a group (q is a compile-time constant after unrolling)
+    __device__ __forceinline__ float group_step(const Group &gr, int q)
+    {
+        const float v = lfib_add(*gr.a[q], *gr.b[q]);
+        *gr.w[q] = v;
+        __syncthreads();
+        return v;
+    }
     __device__ __forceinline__ void store(const Gen &, uint64_t)
     {
         for (int i = threadIdx.x; i < R; i += LFIB_T) st[i] = ring[(pos - R + i) & (RB - 1)];

@@ -65,6 +65,11 @@ N1_LCG32_DRAW = FillCfg("N1_lcg32_2^22x256", LCG32, 1 << 22, 256)
 N1_LCG64_DRAW = FillCfg("N1_lcg64_2^22x256", LCG64, 1 << 22, 256)
 N1_LCG64BOTH_DRAW = FillCfg("N1_lcg64both_2^22x256", LCG64_BOTH, 1 << 22, 256)
 N1_LCG64BOTH = FillCfg("N1_lcg64both_2^20x1024", LCG64_BOTH, 1 << 20, 1024)
+# the float lagged Fibonacci generators (Table 2), same shapes
+N4_LFIB521 = FillCfg("N4_lfib521_2^20x1024", LFIB521, 1 << 20, 1024)
+N4_LFIB1279 = FillCfg("N4_lfib1279_2^20x1024", LFIB1279, 1 << 20, 1024)
+N4_LFIB521_DRAW = FillCfg("N4_lfib521_2^22x256", LFIB521, 1 << 22, 256)
+N4_LFIB1279_DRAW = FillCfg("N4_lfib1279_2^22x256", LFIB1279, 1 << 22, 256)
 
 # C5a: L=4, beta=0.3 vs exact enumeration; 8 streams (K = 1 site per stream per colour)
 C5A_PHILOX = IsingCfg("C5a_ising_L4_philox", PHILOX4X32_10, 4, 0.3, 8, 1000)
