@@ -317,6 +317,16 @@ __global__ void __launch_bounds__(256) lcg_intra_fill_kernel(Gen g, uint32_t *__
     const uint64_t x0 = xs[s];
     const Affine step = tab->pow2[0], leap = tab->pow2[10];
     uint64_t x = affine_apply(tab->mult4[t], x0); // x_{4t}
+    // The stream's final state x_n = step^n(x_0) depends on x_0 only: the last warp computes and stores it
+    // NOW (after every lane has read x_0), so that its dependent table loads overlap the other warps' stores
+    // instead of trailing the CTA.
+    __syncthreads();
+    if (t == 255u) {
+        uint64_t y = x0;
+        for (int m = 0; m < 64 && (n >> m) != 0ull; m++)
+            if ((n >> m) & 1ull) y = affine_apply(tab->pow2[m], y);
+        xs[s] = y;
+    }
     uint32_t *row = out + s * n;
     const bool vec_ok = (n & 3ull) == 0ull;
     for (uint64_t j = 4ull * t; j < n; j += 1024ull) {
@@ -338,13 +348,6 @@ __global__ void __launch_bounds__(256) lcg_intra_fill_kernel(Gen g, uint32_t *__
             if (j + 3 < n) row[j + 3] = v.w;
         }
         x = affine_apply(leap, x);
-    }
-    __syncthreads(); // every lane has read xs[s]
-    if (t == 0) {
-        uint64_t y = x0;
-        for (int m = 0; m < 64 && (n >> m) != 0ull; m++)
-            if ((n >> m) & 1ull) y = affine_apply(tab->pow2[m], y);
-        xs[s] = y;
     }
 }
 
