@@ -106,8 +106,8 @@ __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_
 #pragma unroll
     for (int u = 0; u < U; u++) {
         if (!CHECK || rb0 + 32u * u < blocks_per_row) {
-            const uint4 v = make_uint4(out_word(c0[u], F32), out_word(c1[u], F32), out_word(c2[u], F32),
-                                       out_word(c3[u], F32));
+            const uint4 v = make_uint4(out_word_cvt(c0[u], F32), out_word_cvt(c1[u], F32), out_word_cvt(c2[u], F32),
+                                       out_word_cvt(c3[u], F32));
             __stcs(dst + 32 * u, v); // streaming 128-bit store
         }
     }
@@ -163,8 +163,8 @@ __device__ __forceinline__ void philox_group_fast(uint32_t *__restrict__ row, ui
     uint4 *dst = reinterpret_cast<uint4 *>(row) + rb0;
 #pragma unroll
     for (int u = 0; u < U; u++) {
-        const uint4 v = make_uint4(out_word(c0[u], F32), out_word(c1[u], F32), out_word(c2[u], F32),
-                                   out_word(c3[u], F32));
+        const uint4 v = make_uint4(out_word_cvt(c0[u], F32), out_word_cvt(c1[u], F32), out_word_cvt(c2[u], F32),
+                                   out_word_cvt(c3[u], F32));
         __stcs(dst + 32 * u, v);
     }
 }
