@@ -152,3 +152,86 @@ def test_c5b_ising_L8192_full_lattice(cfg):
     if g.state_bytes():
         assert np.array_equal(g.get_state(), o.get_state())
     g.close()
+
+
+# ---- the widened rows at the sizes bench.py times ------------------------------
+@pytest.mark.parametrize("cfg", [W.N1_PHILOX7, W.N1_LCG32, W.N1_LCG64BOTH, W.N4_LFIB521, W.N4_LFIB1279],
+                         ids=lambda c: c.name)
+def test_next_kinds_4gib_fills_on_sampled_rows(cfg, big_buffer):
+    g = pkg.Rng(cfg.kind, cfg.n_streams, cfg.seed)
+    shards = sample_shards(cfg.n_streams, 256, 6, 4)      # whole lagged Fibonacci instances
+    big_buffer.zero_()
+    g.fill_u32(big_buffer, cfg.n_per_stream)
+    check_fill_rows(cfg, big_buffer, 1, 256, shards)
+    g.fill_f32(big_buffer.view(torch.float32), cfg.n_per_stream)
+    check_fill_rows(cfg, big_buffer, 2, 256, shards, f32=True)
+    g.close()
+
+
+@pytest.mark.parametrize("cfg", [W.N1_PHILOX10_DRAW, W.N1_PHILOX7_DRAW, W.N1_LCG64_DRAW, W.N1_LCG32_DRAW,
+                                 W.N1_LCG64BOTH_DRAW, W.N4_LFIB521_DRAW, W.N4_LFIB1279_DRAW], ids=lambda c: c.name)
+def test_next_kinds_draw_reduce_full(cfg, big_buffer):
+    g = pkg.Rng(cfg.kind, cfg.n_streams, cfg.seed)
+    g.draw_reduce(big_buffer, cfg.n_per_stream)
+    red = big_buffer[:2 * cfg.n_streams].cpu().numpy().view(np.uint32).reshape(-1, 2)
+    m = 256
+    for f in sample_shards(cfg.n_streams, m, 8, 5):
+        o = oracle.Rng(cfg.kind, m, cfg.seed, first=f, n_total=cfg.n_streams)
+        assert np.array_equal(red[f:f + m].reshape(-1), o.draw_reduce(cfg.n_per_stream)), f
+    g.close()
+
+
+def test_skip_ahead_seeding_of_2_19_instances():
+    """C4's 2^24 streams seeded the paper's way: 19 levels of the doubling tree.  Sampled instances against
+    X_0 J^g from the oracle's matrix powers (binary exponentiation over J_k = M^(2^(137+k)))"""
+    S, seed = 1 << 24, W.MASTER_SEED
+    g = pkg.Rng(pkg.RNG_XS1024W_SKIP, S, seed)
+    st = g.get_state().reshape(-1, 32)
+    x0 = oracle.Rng(oracle.XS1024W, 32, seed).get_state()
+    Jk = [oracle.xs1024_matpow2(137)]
+    for _ in range(18):
+        Jk.append(oracle.xs1024_matmul(Jk[-1], Jk[-1]))
+
+    def inst(G):
+        X = x0
+        for k in range(19):
+            if (G >> k) & 1:
+                X = oracle.xs1024_vecmat(X, Jk[k])
+        return X
+    rng = np.random.default_rng(6)
+    for G in [0, 1, 2, (1 << 19) - 1, 1 << 18, (1 << 18) - 1, 0x55555, 0x2AAAA] + rng.integers(0, 1 << 19, 12).tolist():
+        assert np.array_equal(st[G], inst(int(G))), G
+    # the generator itself then runs as kind 4: a draw-mode call on the whole handle, sampled against the oracle
+    # started from those states is covered by test_c4_*; here the first draws of two far-apart instances
+    out = torch.empty(S * 4, dtype=torch.int32, device="cuda")
+    g.fill_u32(out, 4)
+    rows = out.cpu().numpy().view(np.uint32).reshape(S, 4)
+    for G in (0, (1 << 19) - 1):
+        X = inst(G).copy()
+        for j in range(4):
+            oracle.xs1024_update(X)
+            y = (362437 * (j + 1)) & 0xFFFFFFFF
+            assert np.array_equal(rows[32 * G:32 * G + 32, j], ((y ^ (y >> 16)) + X.astype(np.uint64)).astype(np.uint32))
+    g.close()
+
+
+@pytest.mark.parametrize("cfg", [W.T1_XORWOW_K100, W.T1_XORWOW_K1, W.T1_PHILOX_K100, W.T1_XS1024_K100,
+                                 W.T1_XORWOW_K100_T8], ids=lambda c: c.name)
+def test_table1_multihit_L1024_full_lattice(cfg):
+    """the paper's Table-1 workload (1024^2, beta = 0.4, double checkerboard, 262144 streams): the whole lattice
+    and the energy after 1 + 1 sweeps (k = 100: 2 * 10^8 updates on the oracle)"""
+    L = cfg.L
+    g, o = pkg.Rng(cfg.kind, cfg.n_streams, cfg.seed), oracle.Rng(cfg.kind, cfg.n_streams, cfg.seed)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, cfg.lattice_seed)
+    ref = oracle.ising_init_random(L, cfg.lattice_seed)
+    for _ in range(2):
+        tr = torch.empty(1, dtype=torch.int64, device="cuda")
+        g.ising_sweep_multihit(sp, L, cfg.beta, 1, cfg.tile, cfg.k_hits, tr)
+        tr_o = o.ising_sweep_multihit(ref, L, cfg.beta, 1, cfg.tile, cfg.k_hits, trace=True)
+        assert np.array_equal(sp.cpu().numpy(), ref)
+        assert int(tr.item()) == int(tr_o[0])
+    assert g.draws_done == o.draws_done == 8 * cfg.k_hits
+    if g.state_bytes():
+        assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
