@@ -57,6 +57,21 @@ def measured_traffic(name: str):
         return None
 
 
+def measured_ncu(name: str):
+    """ncu-measured utilisation of the workload's dominant kernel from the same committed capture: issue slots,
+    alu / fma / lsu pipes (pct of peak sustained), fma-heavy pipe cycles, DRAM throughput; None if not captured"""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        e = json.load(open(p)).get(name)
+        if not e:
+            return None
+        keys = ("kernel", "ncu_time_us", "issue_active_pct", "pipe_alu_pct", "pipe_fma_pct",
+                "pipe_fmaheavy_cycles_pct_of_elapsed", "pipe_lsu_pct", "dram_throughput_pct", "source")
+        return {k: e.get(k) for k in keys}
+    except Exception:
+        return None
+
+
 def issue_peak_tinst(sm_mhz: float) -> float:
     """thread-instruction issue peak in Tinst/s ('alu' roofline)"""
     return N_SM * SMSP_PER_SM * LANES * sm_mhz * 1e6 / 1e12
@@ -351,6 +366,7 @@ def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, 
         res["roofline"] = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tinst/s", "frac": ach / peak,
                            "traffic": measured_traffic(job.name),
                            "peak_source": "148 SM x 4 SMSP x 32 lanes x sm_max_mhz (issue slots; DESIGN.md s7)"}
+    res["roofline"]["ncu"] = measured_ncu(job.name)
     if clocks:
         res["clocks"] = clocks
     if job.name in PAPER_GTX480:
