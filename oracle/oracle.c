@@ -216,6 +216,7 @@ struct orc_rng {
     uint64_t draws_done;  /* per stream, all streams in lockstep */
     uint64_t *lcg;        /* LCG64: x of each local stream */
     uint64_t leap_X;      /* LEAPFROG: X_{draws_done * n_total} of the global sequence */
+    uint32_t leap_X32;    /* LCG32_LEAPFROG: the same for the 32-bit LCG */
     uint32_t *xw;         /* XORWOW: [n_local][6] */
     uint32_t *xs;         /* XS1024W: [n_local/32][32], word i of instance g at 32 g + i */
     uint32_t *lcg32;      /* LCG32: x of each local stream */
@@ -260,7 +261,7 @@ uint32_t orc_lcg32_step(uint32_t x) { return 1664525u * x + 1013904223u; }
 orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local, uint64_t seed)
 {
     if (n_local < 1 || first + n_local > n_total || first + n_local < first) return NULL;
-    if (kind < ORC_LCG64 || kind > ORC_LFIB1279) return NULL;
+    if (kind < ORC_LCG64 || kind > ORC_LCG32_LEAPFROG) return NULL;
     if ((kind == ORC_LFIB521 || kind == ORC_LFIB1279) && (first % ORC_LFIB_T || n_local % ORC_LFIB_T)) return NULL;
     if ((kind == ORC_XS1024W || kind == ORC_XS1024W_SKIP) && (first % 32 || n_local % 32)) return NULL;
     orc_rng *r = (orc_rng *)calloc(1, sizeof *r);
@@ -274,6 +275,9 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
         break;
     case ORC_LCG64_LEAPFROG: /* sub-streams of ONE sequence: X_0 = SM_seed[0] */
         r->leap_X = orc_splitmix64(seed, 0);
+        break;
+    case ORC_LCG32_LEAPFROG: /* the same for the 32-bit LCG (Table 1 row "LCG32"): X_0 = lo32(SM_seed[0]) */
+        r->leap_X32 = (uint32_t)orc_splitmix64(seed, 0);
         break;
     case ORC_XORWOW: /* R-B2: (x,y),(z,w),(v,d) = (lo,hi) of SM_seed[3s], [3s+1], [3s+2] */
         r->xw = (uint32_t *)malloc(n_local * 6 * sizeof(uint32_t));
@@ -433,6 +437,17 @@ void orc_fill_u32(orc_rng *r, uint32_t *out, uint64_t n)
         r->leap_X = X;
         break;
     }
+    case ORC_LCG32_LEAPFROG: {
+        /* as ORC_LCG64_LEAPFROG: walk the ONE global 32-bit sequence in order; the whole word is the draw */
+        uint32_t X = r->leap_X32;
+        for (uint64_t j = 0; j < n; j++)
+            for (uint64_t m = 0; m < r->n_total; m++) {
+                if (m >= r->first && m < r->first + S) out[(m - r->first) * n + j] = X;
+                X = orc_lcg32_step(X);
+            }
+        r->leap_X32 = X;
+        break;
+    }
     case ORC_XORWOW:
 #pragma omp parallel for schedule(static)
         for (uint64_t s = 0; s < S; s++)
@@ -533,7 +548,7 @@ uint64_t orc_state_words32(const orc_rng *r)
     case ORC_LCG64: case ORC_LCG64_BOTH: case ORC_LCG64_LEAPFROG: return 2 * r->n_local;
     case ORC_XORWOW: return 6 * r->n_local;
     case ORC_XS1024W: case ORC_XS1024W_SKIP: return r->n_local;
-    case ORC_LCG32: return r->n_local;
+    case ORC_LCG32: case ORC_LCG32_LEAPFROG: return r->n_local;
     case ORC_LFIB521: return r->n_local / ORC_LFIB_T * 521;
     case ORC_LFIB1279: return r->n_local / ORC_LFIB_T * 1279;
     default: return 0;
@@ -549,6 +564,14 @@ void orc_get_state(const orc_rng *r, uint32_t *out)
         for (uint64_t m = 0; m < r->first + r->n_local; m++) {
             if (m >= r->first) memcpy(out + 2 * (m - r->first), &X, 8);
             X = orc_lcg64_step(X);
+        }
+        break;
+    }
+    case ORC_LCG32_LEAPFROG: {
+        uint32_t X = r->leap_X32;
+        for (uint64_t m = 0; m < r->first + r->n_local; m++) {
+            if (m >= r->first) out[m - r->first] = X;
+            X = orc_lcg32_step(X);
         }
         break;
     }

@@ -41,7 +41,8 @@ enum {
     ORC_LCG64_BOTH     = 8, /* LCG64 "using the whole state to produce two
                                32-bit numbers": draw 2i = hi32(x_i), draw 2i+1 = lo32(x_i) */
     ORC_LFIB521        = 9, /* PAPER.md:105-124 eq.(5): u_n = u_{n-r} + u_{n-s} mod 1 in float,   */
-    ORC_LFIB1279       = 10 /* (r,s) = (521,353) / (1279,861); ring shared by 256 streams        */
+    ORC_LFIB1279       = 10, /* (r,s) = (521,353) / (1279,861); ring shared by 256 streams       */
+    ORC_LCG32_LEAPFROG = 11  /* kind 1's sub-stream method for the 32-bit LCG (Table 1 row "LCG32") */
 };
 
 /* ---- elementary pieces, exported so that the tests can pin them ---------- */

@@ -99,3 +99,23 @@ def test_lcg64_both_words_is_the_64_bit_sequence_cut_in_two():
     assert [int(v) for v in st] == [oracle.splitmix64(seed, s) for s in range(S)]
     r.fill_u32(1)
     assert [int(v) for v in r.get_state().view(np.uint64)] == [(a * oracle.splitmix64(seed, s) + c) % m for s in range(S)]
+
+
+def test_lcg32_leapfrog_is_one_global_32_bit_sequence():
+    # PAPER.md:39-46 (eq.(2),(3)) applied to the 32-bit LCG, the paper's Table 1 row "LCG32":
+    # all streams draw from ONE sequence x_{m+1} = 1664525 x_m + 1013904223 mod 2^32, stream s draw j = x_{s + j S}.
+    S, n, seed = 7, 9, 4
+    out = oracle.Rng(oracle.LCG32_LEAPFROG, S, seed).fill_u32(n).reshape(S, n)
+    x = oracle.splitmix64(seed, 0) & 0xFFFFFFFF
+    seq = []
+    for _ in range(S * n):
+        seq.append(x)
+        x = (1664525 * x + 1013904223) % (1 << 32)
+    assert np.array_equal(out.T.reshape(-1), np.array(seq, dtype=np.uint32))
+    # shards and continuation see the same sequence; the state is the stream's next element
+    r = oracle.Rng(oracle.LCG32_LEAPFROG, 3, seed, first=2, n_total=S)
+    a, b = r.fill_u32(4).reshape(3, 4), r.fill_u32(5).reshape(3, 5)
+    assert np.array_equal(np.concatenate([a, b], axis=1), out[2:5])
+    r2 = oracle.Rng(oracle.LCG32_LEAPFROG, S, seed)
+    r2.fill_u32(2)
+    assert [int(v) for v in r2.get_state()] == seq[2 * S:3 * S]
