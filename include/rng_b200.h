@@ -114,7 +114,11 @@ enum {
      * as float bit patterns.  Plain ising_sweep only (byte kernel); ising_sweep_multihit
      * returns RNG_E_UNSUPPORTED. */
     RNG_LFIB521 = 9,
-    RNG_LFIB1279 = 10
+    RNG_LFIB1279 = 10,
+    /* kind 1's sub-stream method for the 32-bit LCG of kind 6: ONE global sequence
+     * X_0 = lo32(SM_seed[0]), stream s draw j = X_{s + j*n_total} (the whole word).  This is the paper's
+     * Table 1 row "LCG32", its example of a generator that fails the application test. */
+    RNG_LCG32_LEAPFROG = 11
 };
 
 enum {

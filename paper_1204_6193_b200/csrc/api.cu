@@ -73,7 +73,8 @@ uint64_t rng_state_bytes(int kind, uint64_t n)
     case RNG_XORWOW: return 24 * n;
     case RNG_XS1024W:
     case RNG_XS1024W_SKIP:
-    case RNG_LCG32: return 4 * n;
+    case RNG_LCG32:
+    case RNG_LCG32_LEAPFROG: return 4 * n;
     case RNG_LFIB521: return 4ull * 521ull * (n / 256);
     case RNG_LFIB1279: return 4ull * 1279ull * (n / 256);
     default: return 0;
@@ -84,7 +85,7 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
 {
     if (!out) return fail(RNG_E_INVAL, "rng_create: out is NULL");
     *out = nullptr;
-    if (kind < RNG_LCG64 || kind > RNG_LFIB1279) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
+    if (kind < RNG_LCG64 || kind > RNG_LCG32_LEAPFROG) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
     if (n_local < 1 || first + n_local < first || first + n_local > n_total)
         return fail(RNG_E_INVAL, "rng_create: stream range [%llu,+%llu) not inside [0,%llu)", (unsigned long long)first,
                     (unsigned long long)n_local, (unsigned long long)n_total);
@@ -116,7 +117,8 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
     cudaError_t e = cudaSuccess;
     LcgTable *tab = nullptr;
     if (h->state_bytes) e = cudaMalloc(&h->g.state, h->state_bytes);
-    if (e == cudaSuccess && (kind == RNG_LCG64 || kind == RNG_LCG64_LEAPFROG)) e = cudaMalloc(&tab, sizeof(LcgTable));
+    if (e == cudaSuccess && (kind == RNG_LCG64 || kind == RNG_LCG64_LEAPFROG || kind == RNG_LCG32_LEAPFROG))
+        e = cudaMalloc(&tab, sizeof(LcgTable));
     h->g.lcg = tab;
     if (e == cudaSuccess) e = cudaMalloc(&h->energy_scratch, sizeof(int64_t));
     if (e == cudaSuccess)

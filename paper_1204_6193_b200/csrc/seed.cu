@@ -46,6 +46,22 @@ __global__ void seed_lcg32_kernel(uint32_t *x, uint64_t S, uint64_t first, uint6
     if (s < S) x[s] = (uint32_t)splitmix64_at(seed, first + s);
 }
 
+// RNG_LCG32_LEAPFROG: the step map (a,c)^stride and every stream's origin X_s = (a,c)^(first+s) X_0, all mod 2^32,
+// by binary exponentiation of the affine map (eq.(2),(3); the 64-bit arithmetic truncated)
+__global__ void seed_lcg32_leapfrog_kernel(uint32_t *x, LcgTable *tab, uint64_t S, uint64_t first, uint64_t stride,
+                                           uint64_t seed)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const Affine base{(uint64_t)kLcg32A, (uint64_t)kLcg32C};
+    if (s == 0) {
+        const Affine st = affine_pow(base, stride);
+        tab->pow2[0] = Affine{st.A & 0xffffffffull, st.C & 0xffffffffull};
+    }
+    if (s >= S) return;
+    const Affine j = affine_pow(base, first + s); // mod 2^64; its low 32 bits are the map mod 2^32
+    x[s] = (uint32_t)(j.A * (splitmix64_at(seed, 0) & 0xffffffffull) + j.C);
+}
+
 // RNG_LCG64_LEAPFROG: one global sequence X_0 = SM_seed[0]; stream s starts at X_s =
 // (a,c)^s applied to X_0 -- eq.(2) with t = s, by binary exponentiation.
 __global__ void seed_lcg64_leapfrog_kernel(uint64_t *x, uint64_t S, uint64_t first, uint64_t seed)
@@ -117,6 +133,10 @@ cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st)
         break;
     case RNG_XS1024W:
         seed_xs1024_kernel<<<grid, B, 0, st>>>((uint32_t *)g.state, g.S, g.first, g.seed);
+        count_launch();
+        break;
+    case RNG_LCG32_LEAPFROG:
+        seed_lcg32_leapfrog_kernel<<<grid, B, 0, st>>>((uint32_t *)g.state, tab, g.S, g.first, g.n_total, g.seed);
         count_launch();
         break;
     case RNG_LCG32:

@@ -96,6 +96,25 @@ struct Stream<RNG_LCG32> {
     __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint32_t *)g.state)[s] = x; }
 };
 
+// ---- sub-streams of ONE 32-bit LCG sequence: x <- A x + C with (A, C) = (a, c)^n_total mod 2^32 ----
+template <>
+struct Stream<RNG_LCG32_LEAPFROG> {
+    uint32_t x, A, Cc;
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s)
+    {
+        x = ((const uint32_t *)g.state)[s];
+        A = (uint32_t)g.lcg->pow2[0].A; // built by the seeding kernel (eq.(2))
+        Cc = (uint32_t)g.lcg->pow2[0].C;
+    }
+    __device__ __forceinline__ uint32_t next()
+    {
+        const uint32_t r = x;
+        x = A * x + Cc;
+        return r;
+    }
+    __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint32_t *)g.state)[s] = x; }
+};
+
 // ---- Philox4x32-R: key = global stream id ^ seed; position = draws_done (R-C2) ----
 template <int R>
 struct StreamPhilox {

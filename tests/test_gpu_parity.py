@@ -631,3 +631,14 @@ def test_lfib_ring_wraps_many_times_and_state_round_trips(kind):
     tr_o = o.ising_sweep(sp_o, L, 0.4, 6, trace=True)
     assert np.array_equal(sp.cpu().numpy(), sp_o) and np.array_equal(tr.cpu().numpy(), tr_o)
     g.close()
+
+
+@pytest.mark.slow
+def test_table1_lcg32_substreams_fail_like_in_the_paper():
+    """PAPER.md:80 (Table 1, row 'LCG32'): sub-streams of the ONE 32-bit LCG sequence give "highly significant
+    deviations" (PAPER.md:56); the same kind here misses the exact energy by far more than 10 sigma"""
+    from exact_ising import kaufman
+    exact = kaufman(1024, 0.4)
+    e, e_err, _, _ = _table1_run(pkg.RNG_LCG32_LEAPFROG, 1 << 16, sweeps=20000, nb=40)
+    print(f"\nlcg32_leapfrog: e = {e:.7f} +- {e_err:.7f} (exact {-exact['e']:.7f}, {(e + exact['e']) / e_err:+.1f} sigma)")
+    assert abs(e - (-exact["e"])) > 10 * e_err
