@@ -217,6 +217,7 @@ struct orc_rng {
     uint64_t *lcg;        /* LCG64: x of each local stream */
     uint64_t leap_X;      /* LEAPFROG: X_{draws_done * n_total} of the global sequence */
     uint32_t leap_X32;    /* LCG32_LEAPFROG: the same for the 32-bit LCG */
+    uint32_t *mwc;        /* MWC: [n_local][2] = {x, c} */
     uint32_t *xw;         /* XORWOW: [n_local][6] */
     uint32_t *xs;         /* XS1024W: [n_local/32][32], word i of instance g at 32 g + i */
     uint32_t *lcg32;      /* LCG32: x of each local stream */
@@ -255,13 +256,24 @@ static uint32_t splitmix_word32(uint64_t seed, uint64_t w)
     return (w & 1) ? (uint32_t)(z >> 32) : (uint32_t)z;
 }
 
+/* Multiply-with-carry:  x_{n+1} = a x_n + c_n mod m,  c_{n+1} = floor((a x_n + c_n)/m),
+ * m = 2^32, a = 4294967118 ("a standard choice for a single generator instance"; Table 1 row
+ * "MWC, same a": every stream uses this multiplier, only the seeds differ). */
+#define ORC_MWC_A 4294967118ull
+void orc_mwc_step(uint32_t st[2])
+{
+    uint64_t t = ORC_MWC_A * (uint64_t)st[0] + (uint64_t)st[1];
+    st[0] = (uint32_t)t;         /* x_{n+1} */
+    st[1] = (uint32_t)(t >> 32); /* c_{n+1} */
+}
+
 /* G1: 32-bit LCG, eq.(1) with the constants of PAPER.md:46 */
 uint32_t orc_lcg32_step(uint32_t x) { return 1664525u * x + 1013904223u; }
 
 orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local, uint64_t seed)
 {
     if (n_local < 1 || first + n_local > n_total || first + n_local < first) return NULL;
-    if (kind < ORC_LCG64 || kind > ORC_LCG32_LEAPFROG) return NULL;
+    if (kind < ORC_LCG64 || kind > ORC_MWC) return NULL;
     if ((kind == ORC_LFIB521 || kind == ORC_LFIB1279) && (first % ORC_LFIB_T || n_local % ORC_LFIB_T)) return NULL;
     if ((kind == ORC_XS1024W || kind == ORC_XS1024W_SKIP) && (first % 32 || n_local % 32)) return NULL;
     orc_rng *r = (orc_rng *)calloc(1, sizeof *r);
@@ -275,6 +287,18 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
         break;
     case ORC_LCG64_LEAPFROG: /* sub-streams of ONE sequence: X_0 = SM_seed[0] */
         r->leap_X = orc_splitmix64(seed, 0);
+        break;
+    case ORC_MWC: /* R-M1: (x_0, c_0) = (lo32, hi32 mod a) of SM_seed[s]; the two fixed points (0,0) and
+                   * (m-1, a-1) of the map are moved to (1,0) and (m-1, a-2) */
+        r->mwc = (uint32_t *)malloc(n_local * 2 * sizeof(uint32_t));
+        for (uint64_t s = 0; s < n_local; s++) {
+            uint64_t z = orc_splitmix64(seed, first + s);
+            uint32_t x = (uint32_t)z, cc = (uint32_t)((z >> 32) % ORC_MWC_A);
+            if (x == 0 && cc == 0) x = 1;
+            if (x == 0xffffffffu && cc == (uint32_t)(ORC_MWC_A - 1)) cc = (uint32_t)(ORC_MWC_A - 2);
+            r->mwc[2 * s] = x;
+            r->mwc[2 * s + 1] = cc;
+        }
         break;
     case ORC_LCG32_LEAPFROG: /* the same for the 32-bit LCG (Table 1 row "LCG32"): X_0 = lo32(SM_seed[0]) */
         r->leap_X32 = (uint32_t)orc_splitmix64(seed, 0);
@@ -360,7 +384,7 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
 void orc_destroy(orc_rng *r)
 {
     if (!r) return;
-    free(r->lcg); free(r->xw); free(r->xs); free(r->lcg32); free(r->lf); free(r);
+    free(r->lcg); free(r->xw); free(r->xs); free(r->lcg32); free(r->lf); free(r->mwc); free(r);
 }
 
 uint64_t orc_draws_done(const orc_rng *r) { return r->draws_done; }
@@ -437,6 +461,14 @@ void orc_fill_u32(orc_rng *r, uint32_t *out, uint64_t n)
         r->leap_X = X;
         break;
     }
+    case ORC_MWC:
+#pragma omp parallel for schedule(static)
+        for (uint64_t s = 0; s < S; s++)
+            for (uint64_t j = 0; j < n; j++) {
+                out[s * n + j] = r->mwc[2 * s]; /* the draw is x_n (output, then advance: R-A3) */
+                orc_mwc_step(r->mwc + 2 * s);
+            }
+        break;
     case ORC_LCG32_LEAPFROG: {
         /* as ORC_LCG64_LEAPFROG: walk the ONE global 32-bit sequence in order; the whole word is the draw */
         uint32_t X = r->leap_X32;
@@ -545,7 +577,7 @@ void orc_draw_reduce(orc_rng *r, uint32_t *out, uint64_t n)
 uint64_t orc_state_words32(const orc_rng *r)
 {
     switch (r->kind) {
-    case ORC_LCG64: case ORC_LCG64_BOTH: case ORC_LCG64_LEAPFROG: return 2 * r->n_local;
+    case ORC_LCG64: case ORC_LCG64_BOTH: case ORC_LCG64_LEAPFROG: case ORC_MWC: return 2 * r->n_local;
     case ORC_XORWOW: return 6 * r->n_local;
     case ORC_XS1024W: case ORC_XS1024W_SKIP: return r->n_local;
     case ORC_LCG32: case ORC_LCG32_LEAPFROG: return r->n_local;
@@ -575,6 +607,7 @@ void orc_get_state(const orc_rng *r, uint32_t *out)
         }
         break;
     }
+    case ORC_MWC: memcpy(out, r->mwc, r->n_local * 8); break;
     case ORC_XORWOW: memcpy(out, r->xw, r->n_local * 24); break;
     case ORC_XS1024W: case ORC_XS1024W_SKIP: memcpy(out, r->xs, r->n_local * 4); break;
     case ORC_LCG32: memcpy(out, r->lcg32, r->n_local * 4); break;
