@@ -85,14 +85,14 @@ def issue_peak_tinst(sm_mhz: float) -> float:
 # + checksum (2)
 ALG_INST_PER_DRAW = {W.LCG64: 5.0, W.LCG64_LEAPFROG: 5.0, W.XORWOW: 10.0, W.PHILOX4X32_10: 12.0, W.XS1024W: 7.0,
                      W.PHILOX4X32_7: 9.0, W.LCG32: 3.0, W.XS1024W_SKIP: 7.0,
-                     W.LCG64_BOTH: 3.5, W.LFIB521: 8.0, W.LFIB1279: 8.0, W.LCG32_LEAPFROG: 3.0}  # lfib: 2 LDS, add, compare-subtract, STS,
+                     W.LCG64_BOTH: 3.5, W.LFIB521: 8.0, W.LFIB1279: 8.0, W.LCG32_LEAPFROG: 3.0, W.MWC: 3.0}  # lfib: 2 LDS, add, compare-subtract, STS,
 # barrier, 2 checksum
 # multi-spin-coded update: two threshold compares of two instructions each + the bit-sliced
 # neighbour count / flip logic amortised over the 32 sites of a word (about 1), excl. the draw
 ALG_INST_PER_ISING_UPDATE = 5.0
 STATE_BYTES = {W.LCG64: 8, W.LCG64_LEAPFROG: 8, W.XORWOW: 24, W.PHILOX4X32_10: 0, W.XS1024W: 4, W.PHILOX4X32_7: 0,
                W.LCG32: 4, W.XS1024W_SKIP: 4, W.LCG64_BOTH: 8,
-               W.LFIB521: 521 * 4 / 256.0, W.LFIB1279: 1279 * 4 / 256.0, W.LCG32_LEAPFROG: 4}
+               W.LFIB521: 521 * 4 / 256.0, W.LFIB1279: 1279 * 4 / 256.0, W.LCG32_LEAPFROG: 4, W.MWC: 8}
 
 
 # The paper's own numbers (GTX 480) for the workloads that have one: context, not a target.
@@ -105,6 +105,8 @@ PAPER_GTX480 = {
     "N1_philox7_2^22x256_draw_reduce": (41.0, "Gnum/s", "PAPER.md:269"),
     "N1_lcg64_2^22x256_draw_reduce": (46.0, "Gnum/s", "PAPER.md:261"),
     "N1_lcg32_2^22x256_draw_reduce": (58.0, "Gnum/s", "PAPER.md:259"),
+    "N3_mwc_2^22x256_draw_reduce": (44.0, "Gnum/s", "PAPER.md:95, :263"),
+    "T1_multihit_L1024_mwc_k100": (1.0 / 0.0435, "flips/ns", "PAPER.md:84"),
     "N4_lfib521_2^22x256_draw_reduce": (23.0, "Gnum/s", "PAPER.md:264"),
     "N4_lfib1279_2^22x256_draw_reduce": (23.0, "Gnum/s", "PAPER.md:265"),
     "T1_multihit_L1024_xorwow_k1": (1.0 / 0.7956, "flips/ns", "PAPER.md:88"),
@@ -394,6 +396,8 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
         "N1_lcg32_draw": lambda: DrawJob(W.N1_LCG32_DRAW, rank, world, buf),
         "N1_lcg64_draw": lambda: DrawJob(W.N1_LCG64_DRAW, rank, world, buf),
         "N1_lcg64both_draw": lambda: DrawJob(W.N1_LCG64BOTH_DRAW, rank, world, buf),
+        "N3_mwc_draw": lambda: DrawJob(W.N3_MWC_DRAW, rank, world, buf),
+        "T1_mwc_k100": lambda: IsingJob(W.T1_MWC_K100, rank, world, W.T1_MWC_K100.n_sweeps),
         "N1_lcg64both_u32": lambda: FillJob(W.N1_LCG64BOTH, False, rank, world, buf),
         "N4_lfib521_f32": lambda: FillJob(W.N4_LFIB521, True, rank, world, buf),
         "N4_lfib1279_f32": lambda: FillJob(W.N4_LFIB1279, True, rank, world, buf),
@@ -428,7 +432,7 @@ SUITE = [("C2_f32", 20, 3), ("C1_u32", 200, 10), ("C1_f32", 200, 10), ("C1big_u3
          ("C3_draw", 20, 3), ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1),
          ("C5b_xorwow_K8", 1, 1),
          ("N1_philox7_u32", 20, 3), ("N1_lcg32_u32", 20, 3), ("N1_philox7_draw", 20, 3), ("N1_philox10_draw", 20, 3),
-         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3), ("N1_lcg64both_draw", 20, 3), ("N1_lcg64both_u32", 20, 3),
+         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3), ("N1_lcg64both_draw", 20, 3), ("N1_lcg64both_u32", 20, 3), ("N3_mwc_draw", 20, 3), ("T1_mwc_k100", 3, 3),
          ("N4_lfib521_f32", 20, 3), ("N4_lfib1279_f32", 20, 3), ("N4_lfib521_draw", 20, 3), ("N4_lfib1279_draw", 20, 3),
          ("N2_seed_xs1024_random", 5, 3), ("N2_seed_xs1024_skip", 5, 3),
          ("T1_xorwow_k1", 3, 3), ("T1_xorwow_k100", 3, 3), ("T1_philox_k100", 3, 3), ("T1_xs1024skip_k100", 3, 3),
@@ -447,7 +451,7 @@ def oracle_sample_rate(workload: str, target_s: float = 4.0) -> dict:
     cores = oracle.threads()
     if workload.startswith("T1"):
         cfg = {"T1_xorwow_k1": W.T1_XORWOW_K1, "T1_xorwow_k100": W.T1_XORWOW_K100, "T1_philox_k100": W.T1_PHILOX_K100,
-               "T1_xs1024skip_k100": W.T1_XS1024_K100, "T1_lcg32_k100": W.T1_LCG32_K100,
+               "T1_xs1024skip_k100": W.T1_XS1024_K100, "T1_lcg32_k100": W.T1_LCG32_K100, "T1_mwc_k100": W.T1_MWC_K100,
                "T1big_xorwow_k100": W.T1BIG_XORWOW_K100, "T1big_xorwow_k1": W.T1BIG_XORWOW_K1,
                "T1big_xorwow_k100_t8": W.T1BIG_XORWOW_K100_T8, "T1_xorwow_k100_t8": W.T1_XORWOW_K100_T8}[workload]
         L = 1024  # the paper's lattice; for the L = 8192 workloads 1/64 of the area, same tile and hits
@@ -483,7 +487,7 @@ def oracle_sample_rate(workload: str, target_s: float = 4.0) -> dict:
             "N1_philox7_u32": (W.N1_PHILOX7, "fill_u32"), "N1_lcg32_u32": (W.N1_LCG32, "fill_u32"),
             "N1_philox7_draw": (W.N1_PHILOX7_DRAW, "draw_reduce"), "N1_philox10_draw": (W.N1_PHILOX10_DRAW, "draw_reduce"),
             "N1_lcg32_draw": (W.N1_LCG32_DRAW, "draw_reduce"), "N1_lcg64_draw": (W.N1_LCG64_DRAW, "draw_reduce"),
-            "N1_lcg64both_draw": (W.N1_LCG64BOTH_DRAW, "draw_reduce"), "N1_lcg64both_u32": (W.N1_LCG64BOTH, "fill_u32"),
+            "N1_lcg64both_draw": (W.N1_LCG64BOTH_DRAW, "draw_reduce"), "N3_mwc_draw": (W.N3_MWC_DRAW, "draw_reduce"), "N1_lcg64both_u32": (W.N1_LCG64BOTH, "fill_u32"),
             "N4_lfib521_f32": (W.N4_LFIB521, "fill_f32"), "N4_lfib1279_f32": (W.N4_LFIB1279, "fill_f32"),
             "N4_lfib521_draw": (W.N4_LFIB521_DRAW, "draw_reduce"), "N4_lfib1279_draw": (W.N4_LFIB1279_DRAW, "draw_reduce")}
     cfg, call = cfgs[workload]

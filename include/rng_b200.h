@@ -118,7 +118,12 @@ enum {
     /* kind 1's sub-stream method for the 32-bit LCG of kind 6: ONE global sequence
      * X_0 = lo32(SM_seed[0]), stream s draw j = X_{s + j*n_total} (the whole word).  This is the paper's
      * Table 1 row "LCG32", its example of a generator that fails the application test. */
-    RNG_LCG32_LEAPFROG = 11
+    RNG_LCG32_LEAPFROG = 11,
+    /* Multiply-with-carry: x <- a x + c mod 2^32, c <- floor((a x + c) / 2^32), with the
+     * paper's multiplier a = 4294967118 for every stream (Table 1 row "MWC, same a"); the draw is
+     * x_n (output, then advance).  R-M1: (x_0, c_0) = (lo32, hi32 mod a) of SM_seed[s]; the fixed points (0,0)
+     * and (2^32-1, a-1) are moved to (1,0) and (2^32-1, a-2).  State: n_local x {x, c} u32. */
+    RNG_MWC = 12
 };
 
 enum {

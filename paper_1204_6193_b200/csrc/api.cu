@@ -69,7 +69,8 @@ uint64_t rng_state_bytes(int kind, uint64_t n)
     switch (kind) {
     case RNG_LCG64:
     case RNG_LCG64_LEAPFROG:
-    case RNG_LCG64_BOTH: return 8 * n;
+    case RNG_LCG64_BOTH:
+    case RNG_MWC: return 8 * n;
     case RNG_XORWOW: return 24 * n;
     case RNG_XS1024W:
     case RNG_XS1024W_SKIP:
@@ -85,7 +86,7 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
 {
     if (!out) return fail(RNG_E_INVAL, "rng_create: out is NULL");
     *out = nullptr;
-    if (kind < RNG_LCG64 || kind > RNG_LCG32_LEAPFROG) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
+    if (kind < RNG_LCG64 || kind > RNG_MWC) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
     if (n_local < 1 || first + n_local < first || first + n_local > n_total)
         return fail(RNG_E_INVAL, "rng_create: stream range [%llu,+%llu) not inside [0,%llu)", (unsigned long long)first,
                     (unsigned long long)n_local, (unsigned long long)n_total);

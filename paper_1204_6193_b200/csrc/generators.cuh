@@ -31,6 +31,8 @@ struct Affine {
 };
 constexpr uint64_t kLcgA = 2862933555777941757ull;
 constexpr uint64_t kLcgC = 1442695040888963407ull;
+// multiply-with-carry multiplier (a m - 1 is a safe prime, m = 2^32)
+constexpr uint32_t kMwcA = 4294967118u;
 // the 32-bit LCG of PAPER.md:46 (a = 1664525, c = 1013904223, m = 2^32; Table 2 "LCG32")
 constexpr uint32_t kLcg32A = 1664525u;
 constexpr uint32_t kLcg32C = 1013904223u;

@@ -23,6 +23,7 @@ struct LcgTable {
 //   XORWOW           : u32 w[6][S]   (word k of stream s at w[k*S + s]; k = x,y,z,w,v,d)
 //   PHILOX           : none
 //   XS1024W          : u32 w[S]      (word `lane` of instance g at w[32 g + lane])
+//   MWC              : u64 (c << 32 | x)[S]
 //   LCG32 / LEAPFROG : u32 x[S]   (leapfrog: the step map (a,c)^n_total mod 2^32 sits in LcgTable::pow2[0])
 //   LFIB521 / 1279   : float u[S/256][r]  (an instance's last r numbers, oldest first)
 struct Gen {
@@ -66,6 +67,7 @@ struct rng_handle {
     case RNG_LCG32: MACRO(RNG_LCG32); break;                        \
     case RNG_LCG64_BOTH: MACRO(RNG_LCG64_BOTH); break;              \
     case RNG_LCG32_LEAPFROG: MACRO(RNG_LCG32_LEAPFROG); break;      \
+    case RNG_MWC: MACRO(RNG_MWC); break;                            \
     default: return cudaErrorInvalidValue;                          \
     }
 

@@ -46,6 +46,18 @@ __global__ void seed_lcg32_kernel(uint32_t *x, uint64_t S, uint64_t first, uint6
     if (s < S) x[s] = (uint32_t)splitmix64_at(seed, first + s);
 }
 
+// RNG_MWC (R-M1): (x_0, c_0) = (lo32, hi32 mod a) of SM_seed[s], fixed points moved
+__global__ void seed_mwc_kernel(uint64_t *st, uint64_t S, uint64_t first, uint64_t seed)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    const uint64_t z = splitmix64_at(seed, first + s);
+    uint32_t x = (uint32_t)z, c = (uint32_t)(z >> 32) % kMwcA;
+    if (x == 0u && c == 0u) x = 1u;
+    if (x == 0xffffffffu && c == kMwcA - 1u) c = kMwcA - 2u;
+    st[s] = ((uint64_t)c << 32) | x;
+}
+
 // RNG_LCG32_LEAPFROG: the step map (a,c)^stride and every stream's origin X_s = (a,c)^(first+s) X_0, all mod 2^32,
 // by binary exponentiation of the affine map (eq.(2),(3); the 64-bit arithmetic truncated)
 __global__ void seed_lcg32_leapfrog_kernel(uint32_t *x, LcgTable *tab, uint64_t S, uint64_t first, uint64_t stride,
@@ -133,6 +145,10 @@ cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st)
         break;
     case RNG_XS1024W:
         seed_xs1024_kernel<<<grid, B, 0, st>>>((uint32_t *)g.state, g.S, g.first, g.seed);
+        count_launch();
+        break;
+    case RNG_MWC:
+        seed_mwc_kernel<<<grid, B, 0, st>>>((uint64_t *)g.state, g.S, g.first, g.seed);
         count_launch();
         break;
     case RNG_LCG32_LEAPFROG:

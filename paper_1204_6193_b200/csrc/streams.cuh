@@ -96,6 +96,27 @@ struct Stream<RNG_LCG32> {
     __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint32_t *)g.state)[s] = x; }
 };
 
+// ---- multiply-with-carry: one 32x32+32 -> 64 multiply-add per draw ----
+template <>
+struct Stream<RNG_MWC> {
+    uint32_t x, c;
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s)
+    {
+        const uint64_t v = ((const uint64_t *)g.state)[s];
+        x = (uint32_t)v;
+        c = (uint32_t)(v >> 32);
+    }
+    __device__ __forceinline__ uint32_t next()
+    {
+        const uint32_t r = x;
+        const uint64_t t = (uint64_t)kMwcA * x + c; // a x_n + c_n
+        x = (uint32_t)t;                            // mod m
+        c = (uint32_t)(t >> 32);                    // the carry
+        return r;
+    }
+    __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint64_t *)g.state)[s] = ((uint64_t)c << 32) | x; }
+};
+
 // ---- sub-streams of ONE 32-bit LCG sequence: x <- A x + C with (A, C) = (a, c)^n_total mod 2^32 ----
 template <>
 struct Stream<RNG_LCG32_LEAPFROG> {

@@ -9,7 +9,7 @@ from __future__ import annotations
 
 from dataclasses import dataclass
 
-LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP, LCG64_BOTH, LFIB521, LFIB1279, LCG32_LEAPFROG = range(12)
+LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP, LCG64_BOTH, LFIB521, LFIB1279, LCG32_LEAPFROG, MWC = range(13)
 MASTER_SEED = 1                    # "seeded via splitmix64(master seed 1)" (config 1)
 LATTICE_SEED = 2                   # ising_init_random seed
 BETA_C = 0.44068679350977147       # ln(1+sqrt 2)/2 as a double (config 5)
@@ -64,6 +64,7 @@ N1_PHILOX10_DRAW = FillCfg("N1_philox10_2^22x256", PHILOX4X32_10, 1 << 22, 256)
 N1_LCG32_DRAW = FillCfg("N1_lcg32_2^22x256", LCG32, 1 << 22, 256)
 N1_LCG64_DRAW = FillCfg("N1_lcg64_2^22x256", LCG64, 1 << 22, 256)
 N1_LCG64BOTH_DRAW = FillCfg("N1_lcg64both_2^22x256", LCG64_BOTH, 1 << 22, 256)
+N3_MWC_DRAW = FillCfg("N3_mwc_2^22x256", MWC, 1 << 22, 256)  # PAPER.md:62-68; Table 2 row "MWC"
 N1_LCG64BOTH = FillCfg("N1_lcg64both_2^20x1024", LCG64_BOTH, 1 << 20, 1024)
 # the float lagged Fibonacci generators (Table 2), same shapes
 N4_LFIB521 = FillCfg("N4_lfib521_2^20x1024", LFIB521, 1 << 20, 1024)
@@ -86,6 +87,7 @@ T1_XORWOW_K100 = IsingCfg("T1_multihit_L1024_xorwow_k100", XORWOW, 1024, 0.4, 1 
 T1_PHILOX_K100 = IsingCfg("T1_multihit_L1024_philox_k100", PHILOX4X32_10, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
 T1_XS1024_K100 = IsingCfg("T1_multihit_L1024_xs1024skip_k100", XS1024W_SKIP, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
 T1_LCG32_K100 = IsingCfg("T1_multihit_L1024_lcg32_k100", LCG32, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
+T1_MWC_K100 = IsingCfg("T1_multihit_L1024_mwc_k100", MWC, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
 T1BIG_XORWOW_K100 = IsingCfg("T1big_multihit_L8192_xorwow_k100", XORWOW, 8192, 0.4, 1 << 24, 2, tile=16, k_hits=100)
 T1BIG_XORWOW_K1 = IsingCfg("T1big_multihit_L8192_xorwow_k1", XORWOW, 8192, 0.4, 1 << 24, 100, tile=16, k_hits=1)
 T1BIG_XORWOW_K100_T8 = IsingCfg("T1big_multihit_L8192_xorwow_k100_tile8", XORWOW, 8192, 0.4, 1 << 24, 2, tile=8, k_hits=100)

@@ -68,6 +68,7 @@ def test_state_bytes(L):
     assert pkg.rng_state_bytes(pkg.RNG_LFIB521, 512) == 2 * 521 * 4    # one ring of r words per 256 streams
     assert pkg.rng_state_bytes(pkg.RNG_LFIB1279, 256) == 1279 * 4
     assert pkg.rng_state_bytes(pkg.RNG_LCG32_LEAPFROG, 10) == 40
+    assert pkg.rng_state_bytes(pkg.RNG_MWC, 10) == 80                  # 64 bits: (x, c)
     assert pkg.rng_state_bytes(99, 5) == 0
 
 

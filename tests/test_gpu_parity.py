@@ -437,8 +437,9 @@ def _table1_run(kind, S, seed=1, L=1024, beta=0.4, therm=3000, sweeps=200000, nb
 
 @pytest.mark.slow
 @pytest.mark.parametrize("kind,S", [(pkg.RNG_PHILOX4X32_10, 1 << 17), (pkg.RNG_XORWOW, 1 << 11),
-                                    (pkg.RNG_XS1024W, 1 << 14), (pkg.RNG_LCG64, 1 << 16)],
-                         ids=["philox_K4", "xorwow_K256", "xs1024_K32", "lcg64_random_K8"])
+                                    (pkg.RNG_XS1024W, 1 << 14), (pkg.RNG_LCG64, 1 << 16), (pkg.RNG_MWC, 1 << 16),
+                                    (pkg.RNG_LFIB1279, 1 << 14)],
+                         ids=["philox_K4", "xorwow_K256", "xs1024_K32", "lcg64_random_K8", "mwc_same_a_K8", "lfib1279_K32"])
 def test_table1_L1024_beta04_energy_and_specific_heat_within_3_sigma(kind, S):
     """The paper's application test (Table 1), scaled to 2*10^5 sweeps (2*10^11 updates):
     e and C_V of the 1024^2 lattice at beta = 0.4 agree with Kaufman's exact values (which reproduce the
