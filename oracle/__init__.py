@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
 
-LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP, LCG64_BOTH, LFIB521, LFIB1279, LCG32_LEAPFROG, MWC = range(13)
+LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP, LCG64_BOTH, LFIB521, LFIB1279, LCG32_LEAPFROG, MWC, MWC_MULTI = range(14)
 
 
 def build(force: bool = False) -> str:
@@ -26,7 +26,7 @@ def build(force: bool = False) -> str:
     if (not force and os.path.exists(_SO)
             and os.path.getmtime(_SO) >= max(os.path.getmtime(src), os.path.getmtime(hdr))):
         return _SO
-    cmd = ["gcc", "-std=c99", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
+    cmd = ["gcc", "-std=gnu99", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
            "-o", _SO, src, "-lm"]
     subprocess.run(cmd, check=True)
     return _SO
@@ -128,6 +128,16 @@ def xorwow_next(state: np.ndarray) -> int:
     """advances `state` (6 x uint32, in place) and returns the draw."""
     assert state.dtype == np.uint32 and state.size == 6
     return int(lib().orc_xorwow_next(_p(state)))
+
+
+def mwc_multipliers(first: int, count: int) -> np.ndarray:
+    out = np.empty(count, dtype=np.uint32)
+    L = lib()
+    L.orc_mwc_multipliers.restype = C.c_int
+    L.orc_mwc_multipliers.argtypes = [C.c_uint64, C.c_uint64, C.c_void_p]
+    if L.orc_mwc_multipliers(first, count, _p(out)) != 0:
+        raise ValueError("ran out of multipliers")
+    return out
 
 
 def xs1024_matpow2(k: int) -> np.ndarray:

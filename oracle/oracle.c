@@ -217,7 +217,7 @@ struct orc_rng {
     uint64_t *lcg;        /* LCG64: x of each local stream */
     uint64_t leap_X;      /* LEAPFROG: X_{draws_done * n_total} of the global sequence */
     uint32_t leap_X32;    /* LCG32_LEAPFROG: the same for the 32-bit LCG */
-    uint32_t *mwc;        /* MWC: [n_local][2] = {x, c} */
+    uint32_t *mwc;        /* MWC: [n_local][2] = {x, c};  MWC_MULTI: [n_local][3] = {x, c, a} */
     uint32_t *xw;         /* XORWOW: [n_local][6] */
     uint32_t *xs;         /* XS1024W: [n_local/32][32], word i of instance g at 32 g + i */
     uint32_t *lcg32;      /* LCG32: x of each local stream */
@@ -260,11 +260,75 @@ static uint32_t splitmix_word32(uint64_t seed, uint64_t w)
  * m = 2^32, a = 4294967118 ("a standard choice for a single generator instance"; Table 1 row
  * "MWC, same a": every stream uses this multiplier, only the seeds differ). */
 #define ORC_MWC_A 4294967118ull
+static void mwc_step_a(uint32_t st[2], uint32_t a)
+{
+    uint64_t t = (uint64_t)a * (uint64_t)st[0] + (uint64_t)st[1];
+    st[0] = (uint32_t)t;
+    st[1] = (uint32_t)(t >> 32);
+}
 void orc_mwc_step(uint32_t st[2])
 {
     uint64_t t = ORC_MWC_A * (uint64_t)st[0] + (uint64_t)st[1];
     st[0] = (uint32_t)t;         /* x_{n+1} */
     st[1] = (uint32_t)(t >> 32); /* c_{n+1} */
+}
+
+/* ---- per-stream MWC multipliers, PAPER.md:97 -----------------------------------------
+ * "it is possible to systematically generate multipliers by finding the largest safe prime am-1 with a less
+ * than 2^32 (which is just the a = 4294967118 above) and then systematically working one's way down from there
+ * towards smaller multipliers.  To check for primality one uses probabilistic tests such as the Rabin-Miller
+ * algorithm".  Written out: multiplier number k (k = 0, 1, ...) is the (k+1)-th largest a < 2^32 for which both
+ * p = a 2^32 - 1 and (p - 1)/2 are prime.  Primality: trial division by the primes below 60, then Miller-Rabin
+ * with the twelve bases 2..37, which is a PROOF for numbers below 3.3e24 (all candidates are below 2^64). */
+static uint64_t mulmod64(uint64_t a, uint64_t b, uint64_t n) { return (uint64_t)((unsigned __int128)a * b % n); }
+static uint64_t powmod64(uint64_t a, uint64_t e, uint64_t n)
+{
+    uint64_t r = 1;
+    a %= n;
+    while (e) {
+        if (e & 1) r = mulmod64(r, a, n);
+        a = mulmod64(a, a, n);
+        e >>= 1;
+    }
+    return r;
+}
+int orc_is_prime64(uint64_t n)
+{
+    static const uint64_t small[] = {2, 3, 5, 7, 11, 13, 17, 19, 23, 29, 31, 37, 41, 43, 47, 53, 59};
+    static const uint64_t bases[] = {2, 3, 5, 7, 11, 13, 17, 19, 23, 29, 31, 37};
+    if (n < 2) return 0;
+    for (unsigned i = 0; i < sizeof small / sizeof *small; i++)
+        if (n % small[i] == 0) return n == small[i];
+    uint64_t d = n - 1;
+    int r = 0;
+    while ((d & 1) == 0) { d >>= 1; r++; }
+    for (unsigned i = 0; i < sizeof bases / sizeof *bases; i++) {
+        uint64_t x = powmod64(bases[i], d, n);
+        if (x == 1 || x == n - 1) continue;
+        int composite = 1;
+        for (int k = 1; k < r; k++) {
+            x = mulmod64(x, x, n);
+            if (x == n - 1) { composite = 0; break; }
+        }
+        if (composite) return 0;
+    }
+    return 1;
+}
+int orc_mwc_is_multiplier(uint32_t a)
+{
+    uint64_t p = ((uint64_t)a << 32) - 1; /* a m - 1 */
+    return a > 0 && orc_is_prime64((p - 1) / 2) && orc_is_prime64(p);
+}
+/* out[i] = multiplier number first + i, scanning down from 2^32 - 1.  returns 0, or -1 if the candidates run out */
+int orc_mwc_multipliers(uint64_t first, uint64_t count, uint32_t *out)
+{
+    uint64_t k = 0;
+    for (uint64_t a = 0xffffffffull; a >= 1 && k < first + count; a--)
+        if (orc_mwc_is_multiplier((uint32_t)a)) {
+            if (k >= first) out[k - first] = (uint32_t)a;
+            k++;
+        }
+    return k == first + count ? 0 : -1;
 }
 
 /* G1: 32-bit LCG, eq.(1) with the constants of PAPER.md:46 */
@@ -273,7 +337,7 @@ uint32_t orc_lcg32_step(uint32_t x) { return 1664525u * x + 1013904223u; }
 orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local, uint64_t seed)
 {
     if (n_local < 1 || first + n_local > n_total || first + n_local < first) return NULL;
-    if (kind < ORC_LCG64 || kind > ORC_MWC) return NULL;
+    if (kind < ORC_LCG64 || kind > ORC_MWC_MULTI) return NULL;
     if ((kind == ORC_LFIB521 || kind == ORC_LFIB1279) && (first % ORC_LFIB_T || n_local % ORC_LFIB_T)) return NULL;
     if ((kind == ORC_XS1024W || kind == ORC_XS1024W_SKIP) && (first % 32 || n_local % 32)) return NULL;
     orc_rng *r = (orc_rng *)calloc(1, sizeof *r);
@@ -300,6 +364,23 @@ orc_rng *orc_create(int kind, uint64_t n_total, uint64_t first, uint64_t n_local
             r->mwc[2 * s + 1] = cc;
         }
         break;
+    case ORC_MWC_MULTI: { /* Table 1 row "MWC, different a": stream s (global id) uses multiplier number s; seeds as
+                           * ORC_MWC with its own a: (lo32, hi32 mod a_s), fixed points (0,0), (m-1, a_s-1) moved */
+        uint32_t *mult = (uint32_t *)malloc(n_local * sizeof(uint32_t));
+        if (orc_mwc_multipliers(first, n_local, mult) != 0) { free(mult); free(r); return NULL; }
+        r->mwc = (uint32_t *)malloc(n_local * 3 * sizeof(uint32_t));
+        for (uint64_t s = 0; s < n_local; s++) {
+            uint64_t z = orc_splitmix64(seed, first + s);
+            uint32_t a = mult[s], x = (uint32_t)z, cc = (uint32_t)(z >> 32) % a;
+            if (x == 0 && cc == 0) x = 1;
+            if (x == 0xffffffffu && cc == a - 1) cc = a - 2;
+            r->mwc[3 * s] = x;
+            r->mwc[3 * s + 1] = cc;
+            r->mwc[3 * s + 2] = a;
+        }
+        free(mult);
+        break;
+    }
     case ORC_LCG32_LEAPFROG: /* the same for the 32-bit LCG (Table 1 row "LCG32"): X_0 = lo32(SM_seed[0]) */
         r->leap_X32 = (uint32_t)orc_splitmix64(seed, 0);
         break;
@@ -469,6 +550,14 @@ void orc_fill_u32(orc_rng *r, uint32_t *out, uint64_t n)
                 orc_mwc_step(r->mwc + 2 * s);
             }
         break;
+    case ORC_MWC_MULTI:
+#pragma omp parallel for schedule(static)
+        for (uint64_t s = 0; s < S; s++)
+            for (uint64_t j = 0; j < n; j++) {
+                out[s * n + j] = r->mwc[3 * s];
+                mwc_step_a(r->mwc + 3 * s, r->mwc[3 * s + 2]);
+            }
+        break;
     case ORC_LCG32_LEAPFROG: {
         /* as ORC_LCG64_LEAPFROG: walk the ONE global 32-bit sequence in order; the whole word is the draw */
         uint32_t X = r->leap_X32;
@@ -581,6 +670,7 @@ uint64_t orc_state_words32(const orc_rng *r)
     case ORC_XORWOW: return 6 * r->n_local;
     case ORC_XS1024W: case ORC_XS1024W_SKIP: return r->n_local;
     case ORC_LCG32: case ORC_LCG32_LEAPFROG: return r->n_local;
+    case ORC_MWC_MULTI: return 3 * r->n_local;
     case ORC_LFIB521: return r->n_local / ORC_LFIB_T * 521;
     case ORC_LFIB1279: return r->n_local / ORC_LFIB_T * 1279;
     default: return 0;
@@ -608,6 +698,7 @@ void orc_get_state(const orc_rng *r, uint32_t *out)
         break;
     }
     case ORC_MWC: memcpy(out, r->mwc, r->n_local * 8); break;
+    case ORC_MWC_MULTI: memcpy(out, r->mwc, r->n_local * 12); break;
     case ORC_XORWOW: memcpy(out, r->xw, r->n_local * 24); break;
     case ORC_XS1024W: case ORC_XS1024W_SKIP: memcpy(out, r->xs, r->n_local * 4); break;
     case ORC_LCG32: memcpy(out, r->lcg32, r->n_local * 4); break;

@@ -43,7 +43,8 @@ enum {
     ORC_LFIB521        = 9, /* PAPER.md:105-124 eq.(5): u_n = u_{n-r} + u_{n-s} mod 1 in float,   */
     ORC_LFIB1279       = 10, /* (r,s) = (521,353) / (1279,861); ring shared by 256 streams       */
     ORC_LCG32_LEAPFROG = 11, /* kind 1's sub-stream method for the 32-bit LCG (Table 1 row "LCG32") */
-    ORC_MWC            = 12  /* multiply-with-carry, m = 2^32, a = 4294967118 for all streams */
+    ORC_MWC            = 12, /* multiply-with-carry, m = 2^32, a = 4294967118 for all streams */
+    ORC_MWC_MULTI      = 13  /* one safe-prime multiplier per stream, working down from 4294967118 */
 };
 
 /* ---- elementary pieces, exported so that the tests can pin them ---------- */
@@ -78,6 +79,10 @@ void orc_xs1024_vecmat(const uint32_t X[32], const uint32_t *A, uint32_t out[32]
 void orc_xs1024_matmul(const uint32_t *A, const uint32_t *B, uint32_t *out);
 void orc_xs1024_matpow2(unsigned k, uint32_t *out);
 
+/* is a 2^32 - 1 a safe prime; multipliers number first .. first+count-1 counted down from 2^32 - 1 */
+int orc_is_prime64(uint64_t n);
+int orc_mwc_is_multiplier(uint32_t a);
+int orc_mwc_multipliers(uint64_t first, uint64_t count, uint32_t *out);
 /* one multiply-with-carry step on st = {x, c} */
 void orc_mwc_step(uint32_t st[2]);
 
@@ -112,7 +117,7 @@ void orc_draw_reduce(orc_rng *, uint32_t *out, uint64_t n);
  *   PHILOX: nothing (0 words)
  *   XS1024W: n_local x u32 (word `lane` of instance s/32 at index s)
  *   LFIB: per instance (256 streams) the last r numbers, oldest first, as float bits
- *   MWC: n_local x {x, c} u32 */
+ *   MWC: n_local x {x, c} u32;  MWC_MULTI: n_local x {x, c, a} u32 */
 uint64_t orc_state_words32(const orc_rng *);
 void     orc_get_state(const orc_rng *, uint32_t *out);
 

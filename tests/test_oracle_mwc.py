@@ -94,3 +94,41 @@ def test_uniformity():
     cnt = np.bincount((f * 256).astype(np.int64), minlength=256).astype(np.float64)
     chi2 = ((cnt - n / 256) ** 2 / (n / 256)).sum()
     assert 255 - 3 * math.sqrt(510) < chi2 < 255 + 3 * math.sqrt(510), chi2
+
+
+# ---- "MWC, different a": one safe-prime multiplier per stream -----------------------------
+def test_multipliers_are_the_safe_primes_counted_down_from_the_papers_value():
+    mult = [int(a) for a in oracle.mwc_multipliers(0, 120)]
+    assert mult[0] == A                                            # "which is just the a = 4294967118 above"
+    assert mult == sorted(mult, reverse=True) and len(set(mult)) == len(mult)
+    # every listed a qualifies, and NOTHING in between does (Python Miller-Rabin, independent of the C code)
+    ok = lambda a: _is_probable_prime(a * B - 1) and _is_probable_prime((a * B - 2) // 2)  # noqa: E731
+    listed = set(mult)
+    for a in range(mult[-1], B):
+        assert ok(a) == (a in listed), a
+    # random access further down agrees with the scan from the top
+    far = [int(a) for a in oracle.mwc_multipliers(3000, 5)]
+    assert all(ok(a) for a in far) and far == [int(a) for a in oracle.mwc_multipliers(0, 3005)[3000:]]
+
+
+def test_different_a_streams_are_lehmer_generators_with_their_own_modulus():
+    S, seed, n = 40, 5, 60
+    r = oracle.Rng(oracle.MWC_MULTI, S, seed)
+    st0 = r.get_state().reshape(S, 3)
+    mult = oracle.mwc_multipliers(0, S)
+    assert np.array_equal(st0[:, 2], mult)
+    out = r.fill_u32(n).reshape(S, n)
+    for s in range(S):
+        a = int(mult[s])
+        p = a * B - 1
+        z = oracle.splitmix64(seed, s)
+        assert int(st0[s, 0]) == z & 0xFFFFFFFF and int(st0[s, 1]) == (z >> 32) % a
+        v, binv = int(st0[s, 0]) + B * int(st0[s, 1]), pow(B, -1, p)
+        for j in range(n):
+            assert int(out[s, j]) == v % B
+            v = v * binv % p
+    # a shard uses the multipliers of its GLOBAL stream ids; continuation keeps them
+    sh = oracle.Rng(oracle.MWC_MULTI, 8, seed, first=16, n_total=S)
+    assert np.array_equal(sh.get_state().reshape(8, 3)[:, 2], mult[16:24])
+    a1, a2 = sh.fill_u32(25).reshape(8, 25), sh.fill_u32(35).reshape(8, 35)
+    assert np.array_equal(np.concatenate([a1, a2], axis=1), out[16:24])
