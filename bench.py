@@ -85,14 +85,14 @@ def issue_peak_tinst(sm_mhz: float) -> float:
 # + checksum (2)
 ALG_INST_PER_DRAW = {W.LCG64: 5.0, W.LCG64_LEAPFROG: 5.0, W.XORWOW: 10.0, W.PHILOX4X32_10: 12.0, W.XS1024W: 7.0,
                      W.PHILOX4X32_7: 9.0, W.LCG32: 3.0, W.XS1024W_SKIP: 7.0,
-                     W.LCG64_BOTH: 3.5, W.LFIB521: 8.0, W.LFIB1279: 8.0, W.LCG32_LEAPFROG: 3.0, W.MWC: 3.0}  # lfib: 2 LDS, add, compare-subtract, STS,
+                     W.LCG64_BOTH: 3.5, W.LFIB521: 8.0, W.LFIB1279: 8.0, W.LCG32_LEAPFROG: 3.0, W.MWC: 3.0, W.MWC_MULTI: 3.0}  # lfib: 2 LDS, add, compare-subtract, STS,
 # barrier, 2 checksum
 # multi-spin-coded update: two threshold compares of two instructions each + the bit-sliced
 # neighbour count / flip logic amortised over the 32 sites of a word (about 1), excl. the draw
 ALG_INST_PER_ISING_UPDATE = 5.0
 STATE_BYTES = {W.LCG64: 8, W.LCG64_LEAPFROG: 8, W.XORWOW: 24, W.PHILOX4X32_10: 0, W.XS1024W: 4, W.PHILOX4X32_7: 0,
                W.LCG32: 4, W.XS1024W_SKIP: 4, W.LCG64_BOTH: 8,
-               W.LFIB521: 521 * 4 / 256.0, W.LFIB1279: 1279 * 4 / 256.0, W.LCG32_LEAPFROG: 4, W.MWC: 8}
+               W.LFIB521: 521 * 4 / 256.0, W.LFIB1279: 1279 * 4 / 256.0, W.LCG32_LEAPFROG: 4, W.MWC: 8, W.MWC_MULTI: 10}
 
 
 # The paper's own numbers (GTX 480) for the workloads that have one: context, not a target.

@@ -123,7 +123,12 @@ enum {
      * paper's multiplier a = 4294967118 for every stream (Table 1 row "MWC, same a"); the draw is
      * x_n (output, then advance).  R-M1: (x_0, c_0) = (lo32, hi32 mod a) of SM_seed[s]; the fixed points (0,0)
      * and (2^32-1, a-1) are moved to (1,0) and (2^32-1, a-2).  State: n_local x {x, c} u32. */
-    RNG_MWC = 12
+    RNG_MWC = 12,
+    /* kind 12 with ONE MULTIPLIER PER STREAM (Table 1 row "MWC, different a"): global stream s
+     * uses multiplier number s, the (s+1)-th largest a < 2^32 for which a 2^32 - 1 is a safe prime (number 0 is
+     * the paper's 4294967118); rng_create finds them on the device (trial division + Miller-Rabin, bases 2..37).
+     * Seeds as kind 12 with the stream's own a.  State: n_local x {x, c, a} u32 ("64+32 = 96 bits"). */
+    RNG_MWC_MULTI = 13
 };
 
 enum {

@@ -322,12 +322,22 @@ int orc_mwc_is_multiplier(uint32_t a)
 /* out[i] = multiplier number first + i, scanning down from 2^32 - 1.  returns 0, or -1 if the candidates run out */
 int orc_mwc_multipliers(uint64_t first, uint64_t count, uint32_t *out)
 {
-    uint64_t k = 0;
-    for (uint64_t a = 0xffffffffull; a >= 1 && k < first + count; a--)
-        if (orc_mwc_is_multiplier((uint32_t)a)) {
-            if (k >= first) out[k - first] = (uint32_t)a;
-            k++;
-        }
+    /* the candidates are tested independently (in parallel, a chunk at a time) and then counted in order */
+    enum { CHUNK = 1 << 18 };
+    unsigned char *ok = (unsigned char *)malloc(CHUNK);
+    uint64_t k = 0, top = 0xffffffffull;
+    while (k < first + count && top >= 1) {
+        uint64_t nc = top < CHUNK ? top : CHUNK;
+#pragma omp parallel for schedule(dynamic, 1024)
+        for (uint64_t i = 0; i < nc; i++) ok[i] = (unsigned char)orc_mwc_is_multiplier((uint32_t)(top - i));
+        for (uint64_t i = 0; i < nc && k < first + count; i++)
+            if (ok[i]) {
+                if (k >= first) out[k - first] = (uint32_t)(top - i);
+                k++;
+            }
+        top -= nc;
+    }
+    free(ok);
     return k == first + count ? 0 : -1;
 }
 

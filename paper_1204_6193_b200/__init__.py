@@ -7,7 +7,7 @@ package itself only needs ``ctypes``.  There is no CPU fallback: if the shared
 library is missing or no CUDA device is present, calls raise ``RngError``.
 """
 from .binding import (  # noqa: F401
-    RNG_LCG64, RNG_LCG64_LEAPFROG, RNG_XORWOW, RNG_PHILOX4X32_10, RNG_XS1024W, RNG_PHILOX4X32_7, RNG_LCG32, RNG_XS1024W_SKIP, RNG_LCG64_BOTH, RNG_LFIB521, RNG_LFIB1279, RNG_LCG32_LEAPFROG, RNG_MWC,
+    RNG_LCG64, RNG_LCG64_LEAPFROG, RNG_XORWOW, RNG_PHILOX4X32_10, RNG_XS1024W, RNG_PHILOX4X32_7, RNG_LCG32, RNG_XS1024W_SKIP, RNG_LCG64_BOTH, RNG_LFIB521, RNG_LFIB1279, RNG_LCG32_LEAPFROG, RNG_MWC, RNG_MWC_MULTI,
     RNG_OK, RNG_E_INVAL, RNG_E_NOMEM, RNG_E_CUDA, RNG_E_UNSUPPORTED,
     KIND_NAMES, RngError, Rng, lib, library_path, EXPORTS,
     rng_create, rng_create_shard, rng_destroy, rng_fill_u32, rng_fill_f32, rng_draw_reduce,

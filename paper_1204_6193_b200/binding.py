@@ -14,13 +14,13 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "librng_b200.so")
 
-RNG_LCG64, RNG_LCG64_LEAPFROG, RNG_XORWOW, RNG_PHILOX4X32_10, RNG_XS1024W, RNG_PHILOX4X32_7, RNG_LCG32, RNG_XS1024W_SKIP, RNG_LCG64_BOTH, RNG_LFIB521, RNG_LFIB1279, RNG_LCG32_LEAPFROG, RNG_MWC = range(13)
+RNG_LCG64, RNG_LCG64_LEAPFROG, RNG_XORWOW, RNG_PHILOX4X32_10, RNG_XS1024W, RNG_PHILOX4X32_7, RNG_LCG32, RNG_XS1024W_SKIP, RNG_LCG64_BOTH, RNG_LFIB521, RNG_LFIB1279, RNG_LCG32_LEAPFROG, RNG_MWC, RNG_MWC_MULTI = range(14)
 RNG_OK, RNG_E_INVAL, RNG_E_NOMEM, RNG_E_CUDA, RNG_E_UNSUPPORTED = 0, -1, -2, -3, -4
 KIND_NAMES = {RNG_LCG64: "lcg64", RNG_LCG64_LEAPFROG: "lcg64_leapfrog", RNG_XORWOW: "xorwow",
               RNG_PHILOX4X32_10: "philox4x32_10", RNG_XS1024W: "xs1024w",
               RNG_PHILOX4X32_7: "philox4x32_7", RNG_LCG32: "lcg32", RNG_XS1024W_SKIP: "xs1024w_skip",
               RNG_LCG64_BOTH: "lcg64_both", RNG_LFIB521: "lfib521", RNG_LFIB1279: "lfib1279",
-              RNG_LCG32_LEAPFROG: "lcg32_leapfrog", RNG_MWC: "mwc"}
+              RNG_LCG32_LEAPFROG: "lcg32_leapfrog", RNG_MWC: "mwc", RNG_MWC_MULTI: "mwc_multi"}
 
 _u64, _u32, _i32, _vp, _dbl = C.c_uint64, C.c_uint32, C.c_int, C.c_void_p, C.c_double
 

@@ -72,6 +72,7 @@ uint64_t rng_state_bytes(int kind, uint64_t n)
     case RNG_LCG64_BOTH:
     case RNG_MWC: return 8 * n;
     case RNG_XORWOW: return 24 * n;
+    case RNG_MWC_MULTI: return 12 * n;
     case RNG_XS1024W:
     case RNG_XS1024W_SKIP:
     case RNG_LCG32:
@@ -86,7 +87,7 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
 {
     if (!out) return fail(RNG_E_INVAL, "rng_create: out is NULL");
     *out = nullptr;
-    if (kind < RNG_LCG64 || kind > RNG_MWC) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
+    if (kind < RNG_LCG64 || kind > RNG_MWC_MULTI) return fail(RNG_E_INVAL, "rng_create: unknown kind %d", kind);
     if (n_local < 1 || first + n_local < first || first + n_local > n_total)
         return fail(RNG_E_INVAL, "rng_create: stream range [%llu,+%llu) not inside [0,%llu)", (unsigned long long)first,
                     (unsigned long long)n_local, (unsigned long long)n_total);
@@ -125,6 +126,7 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
     if (e == cudaSuccess)
         e = (kind == RNG_XS1024W_SKIP)                       ? launch_seed_xs1024_skip(h->g, 0)
             : (kind == RNG_LFIB521 || kind == RNG_LFIB1279) ? launch_seed_lfib(h->g, 0)
+            : (kind == RNG_MWC_MULTI)                       ? launch_seed_mwc_multi(h->g, 0)
                                                             : launch_seed(h->g, tab, 0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(0);
     if (e != cudaSuccess) {
@@ -373,12 +375,13 @@ int rng_get_state(rng_handle *h, void *h_buf, uint64_t bytes)
     if (!bytes) return RNG_OK;
     if (!h_buf) return fail(RNG_E_INVAL, "rng_get_state: h_buf is NULL");
     CU(cudaDeviceSynchronize());
-    if (h->g.kind == RNG_XORWOW) { // device layout w[k*S+s] -> canonical [s][k]
-        std::vector<uint32_t> tmp(h->g.S * 6);
+    const int wps = h->g.kind == RNG_XORWOW ? 6 : h->g.kind == RNG_MWC_MULTI ? 3 : 0; // words per stream of the SoA kinds
+    if (wps) { // device layout w[k*S+s] -> canonical [s][k]
+        std::vector<uint32_t> tmp(h->g.S * wps);
         CU(cudaMemcpy(tmp.data(), h->g.state, bytes, cudaMemcpyDeviceToHost));
         uint32_t *o = (uint32_t *)h_buf;
         for (uint64_t s = 0; s < h->g.S; s++)
-            for (int k = 0; k < 6; k++) o[6 * s + k] = tmp[k * h->g.S + s];
+            for (int k = 0; k < wps; k++) o[wps * s + k] = tmp[k * h->g.S + s];
     } else {
         CU(cudaMemcpy(h_buf, h->g.state, bytes, cudaMemcpyDeviceToHost));
     }
@@ -392,11 +395,12 @@ int rng_set_state(rng_handle *h, const void *h_buf, uint64_t bytes)
     if (!bytes) return RNG_OK;
     if (!h_buf) return fail(RNG_E_INVAL, "rng_set_state: h_buf is NULL");
     CU(cudaDeviceSynchronize());
-    if (h->g.kind == RNG_XORWOW) {
-        std::vector<uint32_t> tmp(h->g.S * 6);
+    const int wps = h->g.kind == RNG_XORWOW ? 6 : h->g.kind == RNG_MWC_MULTI ? 3 : 0;
+    if (wps) {
+        std::vector<uint32_t> tmp(h->g.S * wps);
         const uint32_t *in = (const uint32_t *)h_buf;
         for (uint64_t s = 0; s < h->g.S; s++)
-            for (int k = 0; k < 6; k++) tmp[k * h->g.S + s] = in[6 * s + k];
+            for (int k = 0; k < wps; k++) tmp[k * h->g.S + s] = in[wps * s + k];
         CU(cudaMemcpy(h->g.state, tmp.data(), bytes, cudaMemcpyHostToDevice));
     } else {
         CU(cudaMemcpy(h->g.state, h_buf, bytes, cudaMemcpyHostToDevice));

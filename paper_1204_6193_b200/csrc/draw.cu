@@ -185,6 +185,7 @@ cudaError_t launch_draw_reduce(const rng_handle &h, uint32_t *d_out, uint64_t n,
     case RNG_LCG32: draw_reduce_kernel<RNG_LCG32><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     case RNG_LCG64_BOTH: draw_reduce_kernel<RNG_LCG64_BOTH><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     case RNG_MWC: draw_reduce_kernel<RNG_MWC><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
+    case RNG_MWC_MULTI: draw_reduce_kernel<RNG_MWC_MULTI><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     case RNG_LCG32_LEAPFROG: draw_reduce_kernel<RNG_LCG32_LEAPFROG><<<(unsigned)grid, 256, 0, st>>>(g, o, n); break;
     case RNG_LFIB521:
     case RNG_LFIB1279: return launch_lfib_draw(g, d_out, n, st); // CTA = instance (lfib.cu)

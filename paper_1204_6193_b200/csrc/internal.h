@@ -24,6 +24,7 @@ struct LcgTable {
 //   PHILOX           : none
 //   XS1024W          : u32 w[S]      (word `lane` of instance g at w[32 g + lane])
 //   MWC              : u64 (c << 32 | x)[S]
+//   MWC_MULTI        : u32 w[3][S]   (x, c and the stream's multiplier a)
 //   LCG32 / LEAPFROG : u32 x[S]   (leapfrog: the step map (a,c)^n_total mod 2^32 sits in LcgTable::pow2[0])
 //   LFIB521 / 1279   : float u[S/256][r]  (an instance's last r numbers, oldest first)
 struct Gen {
@@ -68,6 +69,7 @@ struct rng_handle {
     case RNG_LCG64_BOTH: MACRO(RNG_LCG64_BOTH); break;              \
     case RNG_LCG32_LEAPFROG: MACRO(RNG_LCG32_LEAPFROG); break;      \
     case RNG_MWC: MACRO(RNG_MWC); break;                            \
+    case RNG_MWC_MULTI: MACRO(RNG_MWC_MULTI); break;                \
     default: return cudaErrorInvalidValue;                          \
     }
 
@@ -77,6 +79,8 @@ void count_launch(uint64_t n = 1);
 
 // seed.cu
 cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st);
+// mwc_multi.cu (RNG_MWC_MULTI: multiplier search + seeding; synchronises the stream, frees its scratch)
+cudaError_t launch_seed_mwc_multi(const Gen &g, cudaStream_t st);
 // lfib.cu (RNG_LFIB521 / RNG_LFIB1279: seeding and fill; draws and Ising go through Stream<KIND>)
 cudaError_t launch_seed_lfib(const Gen &g, cudaStream_t st);
 cudaError_t launch_lfib_fill(const Gen &g, void *d_out, uint64_t n, bool f32, cudaStream_t st);

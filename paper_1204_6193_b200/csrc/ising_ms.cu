@@ -448,6 +448,7 @@ cudaError_t launch_ising_ms_half_sweep(const rng_handle &h, uint32_t *planes, ui
         case RNG_LCG32: launch_ms_word<RNG_LCG32>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         case RNG_LCG64_BOTH: launch_ms_word<RNG_LCG64_BOTH>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         case RNG_MWC: launch_ms_word<RNG_MWC>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
+        case RNG_MWC_MULTI: launch_ms_word<RNG_MWC_MULTI>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         case RNG_LCG32_LEAPFROG: launch_ms_word<RNG_LCG32_LEAPFROG>(g, Cp, Np, L, thr, n_words, K, colour, st); break;
         default: return cudaErrorInvalidValue;
         }

@@ -117,6 +117,33 @@ struct Stream<RNG_MWC> {
     __device__ __forceinline__ void store(const Gen &g, uint64_t s) { ((uint64_t *)g.state)[s] = ((uint64_t)c << 32) | x; }
 };
 
+// ---- multiply-with-carry with the stream's own multiplier ----
+template <>
+struct Stream<RNG_MWC_MULTI> {
+    uint32_t x, c, a;
+    __device__ __forceinline__ void load(const Gen &g, uint64_t s)
+    {
+        const uint32_t *w = (const uint32_t *)g.state;
+        x = w[s];
+        c = w[g.S + s];
+        a = w[2 * g.S + s];
+    }
+    __device__ __forceinline__ uint32_t next()
+    {
+        const uint32_t r = x;
+        const uint64_t t = (uint64_t)a * x + c;
+        x = (uint32_t)t;
+        c = (uint32_t)(t >> 32);
+        return r;
+    }
+    __device__ __forceinline__ void store(const Gen &g, uint64_t s)
+    {
+        uint32_t *w = (uint32_t *)g.state;
+        w[s] = x;
+        w[g.S + s] = c; // the multiplier never changes
+    }
+};
+
 // ---- sub-streams of ONE 32-bit LCG sequence: x <- A x + C with (A, C) = (a, c)^n_total mod 2^32 ----
 template <>
 struct Stream<RNG_LCG32_LEAPFROG> {

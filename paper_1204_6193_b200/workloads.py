@@ -9,7 +9,7 @@ from __future__ import annotations
 
 from dataclasses import dataclass
 
-LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP, LCG64_BOTH, LFIB521, LFIB1279, LCG32_LEAPFROG, MWC = range(13)
+LCG64, LCG64_LEAPFROG, XORWOW, PHILOX4X32_10, XS1024W, PHILOX4X32_7, LCG32, XS1024W_SKIP, LCG64_BOTH, LFIB521, LFIB1279, LCG32_LEAPFROG, MWC, MWC_MULTI = range(14)
 MASTER_SEED = 1                    # "seeded via splitmix64(master seed 1)" (config 1)
 LATTICE_SEED = 2                   # ising_init_random seed
 BETA_C = 0.44068679350977147       # ln(1+sqrt 2)/2 as a double (config 5)

@@ -69,6 +69,7 @@ def test_state_bytes(L):
     assert pkg.rng_state_bytes(pkg.RNG_LFIB1279, 256) == 1279 * 4
     assert pkg.rng_state_bytes(pkg.RNG_LCG32_LEAPFROG, 10) == 40
     assert pkg.rng_state_bytes(pkg.RNG_MWC, 10) == 80                  # 64 bits: (x, c)
+    assert pkg.rng_state_bytes(pkg.RNG_MWC_MULTI, 10) == 120           # "64+32 = 96 bits"
     assert pkg.rng_state_bytes(99, 5) == 0
 
 

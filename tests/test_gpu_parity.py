@@ -438,8 +438,10 @@ def _table1_run(kind, S, seed=1, L=1024, beta=0.4, therm=3000, sweeps=200000, nb
 @pytest.mark.slow
 @pytest.mark.parametrize("kind,S", [(pkg.RNG_PHILOX4X32_10, 1 << 17), (pkg.RNG_XORWOW, 1 << 11),
                                     (pkg.RNG_XS1024W, 1 << 14), (pkg.RNG_LCG64, 1 << 16), (pkg.RNG_MWC, 1 << 16),
-                                    (pkg.RNG_LFIB1279, 1 << 14)],
-                         ids=["philox_K4", "xorwow_K256", "xs1024_K32", "lcg64_random_K8", "mwc_same_a_K8", "lfib1279_K32"])
+                                    (pkg.RNG_LFIB1279, 1 << 14), (pkg.RNG_MWC_MULTI, 1 << 16),
+                                    (pkg.RNG_PHILOX4X32_7, 1 << 17)],
+                         ids=["philox_K4", "xorwow_K256", "xs1024_K32", "lcg64_random_K8", "mwc_same_a_K8", "lfib1279_K32",
+                              "mwc_different_a_K8", "philox7_K4"])
 def test_table1_L1024_beta04_energy_and_specific_heat_within_3_sigma(kind, S):
     """The paper's application test (Table 1), scaled to 2*10^5 sweeps (2*10^11 updates):
     e and C_V of the 1024^2 lattice at beta = 0.4 agree with Kaufman's exact values (which reproduce the
@@ -643,3 +645,20 @@ def test_table1_lcg32_substreams_fail_like_in_the_paper():
     e, e_err, _, _ = _table1_run(pkg.RNG_LCG32_LEAPFROG, 1 << 16, sweeps=20000, nb=40)
     print(f"\nlcg32_leapfrog: e = {e:.7f} +- {e_err:.7f} (exact {-exact['e']:.7f}, {(e + exact['e']) / e_err:+.1f} sigma)")
     assert abs(e - (-exact["e"])) > 10 * e_err
+
+
+def test_mwc_multipliers_found_on_the_device_match_the_oracles_scan():
+    """2^16 streams with their own safe-prime multipliers (several chunks of the device search),
+    for a shard that starts in the middle of the list; all of them against the oracle's scan from the top"""
+    first, S = 5000, 1 << 16
+    g = pkg.Rng(pkg.RNG_MWC_MULTI, S, 3, first=first, n_total=first + S)
+    st = g.get_state().reshape(S, 3)
+    want = oracle.mwc_multipliers(first, S)
+    assert np.array_equal(st[:, 2], want)
+    assert int(oracle.mwc_multipliers(0, 1)[0]) == 4294967118            # the paper's multiplier is number 0
+    o = oracle.Rng(pkg.RNG_MWC_MULTI, 512, 3, first=first, n_total=first + S)
+    assert np.array_equal(st[:512].reshape(-1), o.get_state())
+    out = dev_u32(S * 8)
+    g.fill_u32(out, 8)
+    assert np.array_equal(host(out, S * 8).reshape(S, 8)[:512], o.fill_u32(8).reshape(512, 8))
+    g.close()

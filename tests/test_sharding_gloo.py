@@ -31,7 +31,7 @@ def _worker(rank: int, world: int, port: int, n_per_rank: int, n: int):
     try:
         for kind in (W.LCG64, W.LCG64_LEAPFROG, W.XORWOW, W.PHILOX4X32_10, W.XS1024W, W.PHILOX4X32_7, W.LCG32,
                      W.XS1024W_SKIP, W.LCG64_BOTH, W.LFIB521, W.LFIB1279, W.LCG32_LEAPFROG,
-                     W.MWC):
+                     W.MWC, W.MWC_MULTI):
             # bench.py's weak-scaling layout (the lagged Fibonacci kinds come in 256-stream instances)
             per = 256 if kind in (W.LFIB521, W.LFIB1279) else n_per_rank
             n_total, first, n_local = sharding.weak_scaling_shard(rank, world, per)
