@@ -107,6 +107,8 @@ PAPER_GTX480 = {
     "N1_lcg32_2^22x256_draw_reduce": (58.0, "Gnum/s", "PAPER.md:259"),
     "N3_mwc_2^22x256_draw_reduce": (44.0, "Gnum/s", "PAPER.md:95, :263"),
     "T1_multihit_L1024_mwc_k100": (1.0 / 0.0435, "flips/ns", "PAPER.md:84"),
+    "T1_multihit_L1024_lfib521_k100": (1.0 / 0.0661, "flips/ns", "PAPER.md:86"),
+    "T1_multihit_L1024_lfib1279_k100": (1.0 / 0.0700, "flips/ns", "PAPER.md:87"),
     "N4_lfib521_2^22x256_draw_reduce": (23.0, "Gnum/s", "PAPER.md:264"),
     "N4_lfib1279_2^22x256_draw_reduce": (23.0, "Gnum/s", "PAPER.md:265"),
     "T1_multihit_L1024_xorwow_k1": (1.0 / 0.7956, "flips/ns", "PAPER.md:88"),
@@ -398,6 +400,8 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
         "N1_lcg64both_draw": lambda: DrawJob(W.N1_LCG64BOTH_DRAW, rank, world, buf),
         "N3_mwc_draw": lambda: DrawJob(W.N3_MWC_DRAW, rank, world, buf),
         "T1_mwc_k100": lambda: IsingJob(W.T1_MWC_K100, rank, world, W.T1_MWC_K100.n_sweeps),
+        "T1_lfib521_k100": lambda: IsingJob(W.T1_LFIB521_K100, rank, world, W.T1_LFIB521_K100.n_sweeps),
+        "T1_lfib1279_k100": lambda: IsingJob(W.T1_LFIB1279_K100, rank, world, W.T1_LFIB1279_K100.n_sweeps),
         "N1_lcg64both_u32": lambda: FillJob(W.N1_LCG64BOTH, False, rank, world, buf),
         "N4_lfib521_f32": lambda: FillJob(W.N4_LFIB521, True, rank, world, buf),
         "N4_lfib1279_f32": lambda: FillJob(W.N4_LFIB1279, True, rank, world, buf),
@@ -432,7 +436,7 @@ SUITE = [("C2_f32", 20, 3), ("C1_u32", 200, 10), ("C1_f32", 200, 10), ("C1big_u3
          ("C3_draw", 20, 3), ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1),
          ("C5b_xorwow_K8", 1, 1),
          ("N1_philox7_u32", 20, 3), ("N1_lcg32_u32", 20, 3), ("N1_philox7_draw", 20, 3), ("N1_philox10_draw", 20, 3),
-         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3), ("N1_lcg64both_draw", 20, 3), ("N1_lcg64both_u32", 20, 3), ("N3_mwc_draw", 20, 3), ("T1_mwc_k100", 3, 3),
+         ("N1_lcg32_draw", 20, 3), ("N1_lcg64_draw", 20, 3), ("N1_lcg64both_draw", 20, 3), ("N1_lcg64both_u32", 20, 3), ("N3_mwc_draw", 20, 3), ("T1_mwc_k100", 3, 3), ("T1_lfib521_k100", 3, 3), ("T1_lfib1279_k100", 3, 3),
          ("N4_lfib521_f32", 20, 3), ("N4_lfib1279_f32", 20, 3), ("N4_lfib521_draw", 20, 3), ("N4_lfib1279_draw", 20, 3),
          ("N2_seed_xs1024_random", 5, 3), ("N2_seed_xs1024_skip", 5, 3),
          ("T1_xorwow_k1", 3, 3), ("T1_xorwow_k100", 3, 3), ("T1_philox_k100", 3, 3), ("T1_xs1024skip_k100", 3, 3),
@@ -452,6 +456,7 @@ def oracle_sample_rate(workload: str, target_s: float = 4.0) -> dict:
     if workload.startswith("T1"):
         cfg = {"T1_xorwow_k1": W.T1_XORWOW_K1, "T1_xorwow_k100": W.T1_XORWOW_K100, "T1_philox_k100": W.T1_PHILOX_K100,
                "T1_xs1024skip_k100": W.T1_XS1024_K100, "T1_lcg32_k100": W.T1_LCG32_K100, "T1_mwc_k100": W.T1_MWC_K100,
+               "T1_lfib521_k100": W.T1_LFIB521_K100, "T1_lfib1279_k100": W.T1_LFIB1279_K100,
                "T1big_xorwow_k100": W.T1BIG_XORWOW_K100, "T1big_xorwow_k1": W.T1BIG_XORWOW_K1,
                "T1big_xorwow_k100_t8": W.T1BIG_XORWOW_K100_T8, "T1_xorwow_k100_t8": W.T1_XORWOW_K100_T8}[workload]
         L = 1024  # the paper's lattice; for the L = 8192 workloads 1/64 of the area, same tile and hits

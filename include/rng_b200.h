@@ -111,8 +111,8 @@ enum {
      * that bit on u_0.  All values are 23-bit fractions, every addition is exact.  fill_f32
      * writes the numbers themselves; as 32-bit integers they are (v 2^23) << 9, so the fixed
      * map (u >> 8) 2^-24 gives v back.  State: per instance its last r numbers, oldest first,
-     * as float bit patterns.  Plain ising_sweep only (byte kernel); ising_sweep_multihit
-     * returns RNG_E_UNSUPPORTED. */
+     * as float bit patterns.  ising_sweep runs on the byte kernel, ising_sweep_multihit with tile 8 or 16
+     * (a CTA = one instance hosts 256 / (tile*tile/2) tiles). */
     RNG_LFIB521 = 9,
     RNG_LFIB1279 = 10,
     /* kind 1's sub-stream method for the 32-bit LCG of kind 6: ONE global sequence
@@ -197,7 +197,8 @@ int ising_sweep(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_
  * the site y_l = t/(tile/2), x_l = 2*(t%(tile/2)) + ((y_l+c)&1) of the tile; stream
  * s = p*tile*tile/2 + t serves tile p of both coarse colours and spends its draws in the order
  * (coarse colour, hit, fine colour): 4*k_hits per sweep, 2*k_hits per generator state load.
- * RNG_XS1024W / _SKIP need tile % 8 == 0.  d_energy_trace as in ising_sweep.
+ * RNG_XS1024W / _SKIP need tile % 8 == 0; RNG_LFIB* (ring shared by a 256-thread CTA) tile 8 or 16, else
+ * RNG_E_UNSUPPORTED.  d_energy_trace as in ising_sweep.
  * draws_done += 4*k_hits*n_sweeps.  Errors: RNG_E_INVAL (geometry, stream count), RNG_E_CUDA. */
 int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_t n_sweeps,
                          uint32_t tile, uint32_t k_hits, int64_t *d_energy_trace, void *cuda_stream);

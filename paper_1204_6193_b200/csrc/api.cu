@@ -266,8 +266,8 @@ int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta
         return fail(RNG_E_INVAL, "ising_sweep_multihit: tile must be even, 2..44, divide L, with L/tile even");
     if (k_hits < 1) return fail(RNG_E_INVAL, "ising_sweep_multihit: k_hits must be >= 1");
     if (h->g.S != (uint64_t)L * L / 4) return fail(RNG_E_INVAL, "ising_sweep_multihit: needs n_streams == L*L/4");
-    if (h->g.kind == RNG_LFIB521 || h->g.kind == RNG_LFIB1279)
-        return fail(RNG_E_UNSUPPORTED, "ising_sweep_multihit: RNG_LFIB* shares its state across a 256-thread CTA; use ising_sweep");
+    if ((h->g.kind == RNG_LFIB521 || h->g.kind == RNG_LFIB1279) && tile != 8u && tile != 16u)
+        return fail(RNG_E_UNSUPPORTED, "ising_sweep_multihit: RNG_LFIB* shares its ring across a 256-thread CTA: tile 8 or 16 only");
     if (h->g.kind == RNG_XS1024W && (tile * tile / 2u) % 32u)
         return fail(RNG_E_INVAL, "ising_sweep_multihit: this kind needs whole warps per tile (tile a multiple of 8)");
     const uint64_t per_sweep = 4ull * k_hits;

@@ -23,8 +23,11 @@
 
 namespace rngb200 {
 
-// WARP_TILE: tile = 8, a tile is exactly one warp (32 dominoes): a CTA hosts blockDim.x/32 tiles, each in
-// its own slab of shared memory, and the two barriers of a hit are __syncwarp() instead of __syncthreads().
+// A CTA hosts blockDim.x / (T*T/2) tiles, each in its own slab of shared memory (one tile per CTA in the plain case).
+// WARP_TILE: tile = 8, a tile is exactly one warp (32 dominoes) and the two barriers of a hit are __syncwarp()
+// instead of __syncthreads().  The lagged Fibonacci kinds share their ring among the 256 threads of a CTA
+// (lfib.cuh), so their CTA hosts 256 / (T*T/2) tiles (T = 16: two, T = 8: eight) and keeps the block barriers:
+// stream s = p T*T/2 + t is then blockIdx.x*256 + threadIdx.x, the instance <-> CTA map that generator needs.
 template <int KIND, bool WARP_TILE>
 __global__ void ising_multihit_kernel(Gen g, int8_t *__restrict__ sp, uint32_t L, IsingTable tab, uint32_t T,
                                       uint32_t k_hits, uint32_t C, uint32_t n_tiles)
@@ -35,10 +38,12 @@ __global__ void ising_multihit_kernel(Gen g, int8_t *__restrict__ sp, uint32_t L
     for (uint32_t i = threadIdx.x; i < 5u; i += blockDim.x) thr[2u * i] = tab.T[i]; // a 2 x 2 tile has 2 threads
     const uint32_t RS = T + 8u, half = T >> 1;
     // (T+2) rows of RS bytes; interior row y_l at row y_l+1, columns 4 .. 4+T-1, halo columns 3 and 4+T
-    int8_t *tile = mh_smem + 64 + (WARP_TILE ? (threadIdx.x >> 5) * (((T + 2u) * RS + 15u) & ~15u) : 0u);
-    const uint32_t t = WARP_TILE ? (threadIdx.x & 31u) : threadIdx.x;
+    const uint32_t tile_threads = half * T;
+    const uint32_t sub = WARP_TILE ? (threadIdx.x >> 5) : threadIdx.x / tile_threads; // tile of this CTA
+    int8_t *tile = mh_smem + 64 + sub * (((T + 2u) * RS + 15u) & ~15u);
+    const uint32_t t = threadIdx.x - sub * tile_threads;
     const uint32_t nth = (L / T) >> 1;
-    const uint32_t p = WARP_TILE ? blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5) : blockIdx.x;
+    const uint32_t p = blockIdx.x * (blockDim.x / tile_threads) + sub;
     const bool tile_live = p < n_tiles; // warp-uniform; dead warps still take part in the CTA barrier below
     if (WARP_TILE && !tile_live) {
         __syncthreads();
@@ -62,7 +67,7 @@ __global__ void ising_multihit_kernel(Gen g, int8_t *__restrict__ sp, uint32_t L
         tile[(t + 1u) * RS + 3u] = sp[(uint64_t)(y0 + t) * L + xl];
         tile[(t + 1u) * RS + 4u + T] = sp[(uint64_t)(y0 + t) * L + xr];
     }
-    const uint64_t s = (uint64_t)p * (half * T) + t;
+    const uint64_t s = (uint64_t)p * tile_threads + t;
     Stream<KIND> gen;
     gen.load(g, s);
     __syncthreads(); // thresholds and tile(s) are in place
@@ -113,7 +118,15 @@ cudaError_t launch_ising_multihit(const rng_handle &h, int8_t *d_spins, uint32_t
     g.draws_done = draws_done;
     const uint32_t tiles = (L / T) * (L / T) / 2u;
     const size_t slab = ((size_t)(T + 2u) * (T + 8u) + 15u) & ~(size_t)15u;
-    if (T == 8u) { // one warp per tile, four tiles per CTA
+    if (kind_is_lfib(g.kind)) { // CTA = one 256-stream instance = 256 / (T*T/2) tiles (api.cu admits T = 8, 16 only)
+        const uint32_t tpc = 256u / (T * T / 2u), grid = tiles / tpc; // tiles % tpc == 0 because L % 32 == 0
+        if (g.kind == RNG_LFIB1279)
+            ising_multihit_kernel<RNG_LFIB1279, false><<<grid, 256, 64 + tpc * slab, st>>>(g, d_spins, L, tab, T, k_hits,
+                                                                                          (uint32_t)coarse, tiles);
+        else
+            ising_multihit_kernel<RNG_LFIB521, false><<<grid, 256, 64 + tpc * slab, st>>>(g, d_spins, L, tab, T, k_hits,
+                                                                                         (uint32_t)coarse, tiles);
+    } else if (T == 8u) { // one warp per tile, four tiles per CTA
         const uint32_t wpc = 4u, grid = (tiles + wpc - 1u) / wpc;
 #define MH(KIND)                                                                                                  \
     ising_multihit_kernel<KIND, true><<<grid, wpc * 32u, 64 + wpc * slab, st>>>(g, d_spins, L, tab, T, k_hits, \

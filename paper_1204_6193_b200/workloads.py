@@ -88,6 +88,8 @@ T1_PHILOX_K100 = IsingCfg("T1_multihit_L1024_philox_k100", PHILOX4X32_10, 1024, 
 T1_XS1024_K100 = IsingCfg("T1_multihit_L1024_xs1024skip_k100", XS1024W_SKIP, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
 T1_LCG32_K100 = IsingCfg("T1_multihit_L1024_lcg32_k100", LCG32, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
 T1_MWC_K100 = IsingCfg("T1_multihit_L1024_mwc_k100", MWC, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
+T1_LFIB521_K100 = IsingCfg("T1_multihit_L1024_lfib521_k100", LFIB521, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
+T1_LFIB1279_K100 = IsingCfg("T1_multihit_L1024_lfib1279_k100", LFIB1279, 1024, 0.4, 1 << 18, 10, tile=16, k_hits=100)
 T1BIG_XORWOW_K100 = IsingCfg("T1big_multihit_L8192_xorwow_k100", XORWOW, 8192, 0.4, 1 << 24, 2, tile=16, k_hits=100)
 T1BIG_XORWOW_K1 = IsingCfg("T1big_multihit_L8192_xorwow_k1", XORWOW, 8192, 0.4, 1 << 24, 100, tile=16, k_hits=1)
 T1BIG_XORWOW_K100_T8 = IsingCfg("T1big_multihit_L8192_xorwow_k100_tile8", XORWOW, 8192, 0.4, 1 << 24, 2, tile=8, k_hits=100)

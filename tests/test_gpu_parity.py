@@ -535,8 +535,8 @@ def test_ising_multihit_bit_exact(kind, L, T, k, sweeps):
     S = L * L // 4
     if kind in XS_KINDS and (S % 32 or (T * T // 2) % 32):
         pytest.skip("whole warp instances per tile only")
-    if kind in LFIB_KINDS:
-        pytest.skip("CTA-shared state: plain ising_sweep only (RNG_E_UNSUPPORTED is tested below)")
+    if kind in LFIB_KINDS and (S % 256 or T not in (8, 16)):
+        pytest.skip("ring shared by a 256-thread CTA: whole instances, tile 8 or 16 (RNG_E_UNSUPPORTED is tested below)")
     beta = 0.44068679350977147
     g, o = pkg.Rng(kind, S, 13), oracle.Rng(kind, S, 13)
     sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
@@ -567,16 +567,17 @@ def test_ising_multihit_argument_errors():
     with pytest.raises(pkg.RngError):
         g.ising_sweep_multihit(sp, 8, 0.3, 1, 2, 1)
     g.close()
-    g = pkg.Rng(pkg.RNG_LFIB521, 256, 1)               # CTA-shared state does not fit the tile <-> CTA map
-    sp = torch.ones(32 * 32, dtype=torch.int8, device="cuda")
+    g = pkg.Rng(pkg.RNG_LFIB521, 1024, 1)              # a 32 x 32 tile has 512 threads: two instances, not offered
+    sp = torch.ones(64 * 64, dtype=torch.int8, device="cuda")
     with pytest.raises(pkg.RngError) as e:
-        g.ising_sweep_multihit(sp, 32, 0.3, 1, 8, 1)
+        g.ising_sweep_multihit(sp, 64, 0.3, 1, 32, 1)
     assert e.value.code == pkg.RNG_E_UNSUPPORTED
     g.close()
 
 
-@pytest.mark.parametrize("kind", [pkg.RNG_PHILOX4X32_10, pkg.RNG_XORWOW, pkg.RNG_XS1024W_SKIP],
-                         ids=["philox10", "xorwow", "xs1024w_skip"])
+@pytest.mark.parametrize("kind", [pkg.RNG_PHILOX4X32_10, pkg.RNG_XORWOW, pkg.RNG_XS1024W_SKIP, pkg.RNG_LFIB1279,
+                                  pkg.RNG_MWC_MULTI],
+                         ids=["philox10", "xorwow", "xs1024w_skip", "lfib1279", "mwc_different_a"])
 def test_table1_multihit_L1024_beta04_energy_within_3_sigma(kind):
     """the paper's application test with its own kernel shape (Table 1): L = 1024, beta = 0.4,
     double checkerboard, one stream per thread (262144), e and C_V against Kaufman's exact values"""
