@@ -1,6 +1,6 @@
 """Reproduce the paper's Table 1 on one B200 with this library.
 
-    python -m paper_1204_6193_b200.table1 [--sweeps 100000] [--therm 3000] [--tile 16] [--markdown]
+    python -m paper_1204_6193_b200.table1 [--sweeps 100000] [--therm 3000] [--tile 16] [--only KIND,...] [--markdown]
 
 For every generator of the table: a Metropolis simulation of the 1024 x 1024 Ising model at beta = 0.4 with
 the paper's double-checkerboard kernel (ising_sweep_multihit, k = 1, one stream per thread = 262144 streams),
@@ -72,7 +72,9 @@ def main():
     ap.add_argument("--bins", type=int, default=100)
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--markdown", action="store_true")
+    ap.add_argument("--only", default="", help="comma-separated kind names (e.g. RNG_XORWOW,RNG_LFIB521); default: all rows")
     a = ap.parse_args()
+    only = {k.strip() for k in a.only.split(",") if k.strip()}
     import numpy as np
     import torch
 
@@ -86,6 +88,8 @@ def main():
     else:
         print(sep.join(head))
     for label, kname, t1_paper, t100_paper, d_paper in ROWS:
+        if only and kname not in only:
+            continue
         kind = getattr(pkg, kname)
         g = pkg.Rng(kind, L * L // 4, a.seed)
         sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
