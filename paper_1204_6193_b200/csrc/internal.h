@@ -75,6 +75,39 @@ struct rng_handle {
 
 namespace rngb200 {
 
+// Programmatic dependent launch for chains of short, dependent launches (the half-sweeps of a call): with this
+// attribute the next grid is scheduled while the current one drains; the kernels order themselves with
+// pdl_entry() (griddepcontrol.launch_dependents + griddepcontrol.wait, no-ops without the attribute), which must
+// come before their first access to anything the previous launch wrote.  Only worth it when the grid is small:
+// waiting CTAs of a big dependent grid take resources from the grid they wait for (measured: 85 -> 113 flips/ns for
+// the 1024^2 multi-hit k = 1 half-sweeps), so `enable` is false above about one wave of threads.  It is NOT used for
+// the multi-spin half-sweeps of ising_ms.cu: their grids are compute-bound and far from launch-bound, and the
+// waiting CTAs of the next grid cost them 22 % (1796 -> 1404 flips/ns measured).
+struct PdlLaunch {
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    PdlLaunch(dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool enable)
+    {
+        cfg = cudaLaunchConfig_t{};
+        cfg.gridDim = grid;
+        cfg.blockDim = block;
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = enable ? 1u : 0u;
+    }
+};
+constexpr uint64_t kPdlMaxThreads = 148ull * 2048ull; // one wave of resident threads on a B200
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_entry()
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+#endif
+
 void count_launch(uint64_t n = 1);
 
 // seed.cu

@@ -36,6 +36,10 @@ __global__ void ising_multihit_kernel(Gen g, int8_t *__restrict__ sp, uint32_t L
     // thresholds indexed by h + 4 (h = spin * neighbour sum, even): word address = 4 h + const, one IMAD
     uint32_t *thr = reinterpret_cast<uint32_t *>(mh_smem);
     for (uint32_t i = threadIdx.x; i < 5u; i += blockDim.x) thr[2u * i] = tab.T[i]; // a 2 x 2 tile has 2 threads
+    // Programmatic dependent launch: this grid may have been scheduled while the previous half-sweep was still
+    // draining; everything above is independent of it, everything below (spins, generator state) is not.
+    // Let the next launch be scheduled right away: it waits at the same point for THIS grid to complete.
+    pdl_entry();
     const uint32_t RS = T + 8u, half = T >> 1;
     // (T+2) rows of RS bytes; interior row y_l at row y_l+1, columns 4 .. 4+T-1, halo columns 3 and 4+T
     const uint32_t tile_threads = half * T;
@@ -118,30 +122,31 @@ cudaError_t launch_ising_multihit(const rng_handle &h, int8_t *d_spins, uint32_t
     g.draws_done = draws_done;
     const uint32_t tiles = (L / T) * (L / T) / 2u;
     const size_t slab = ((size_t)(T + 2u) * (T + 8u) + 15u) & ~(size_t)15u;
+    // programmatic dependent launch (internal.h) when the grid is at most about one wave
+    const bool pdl = (uint64_t)L * L / 4ull <= kPdlMaxThreads; // one thread per stream of the active colour
+    const uint32_t C = (uint32_t)coarse;
+    cudaError_t e = cudaSuccess;
     if (kind_is_lfib(g.kind)) { // CTA = one 256-stream instance = 256 / (T*T/2) tiles (api.cu admits T = 8, 16 only)
-        const uint32_t tpc = 256u / (T * T / 2u), grid = tiles / tpc; // tiles % tpc == 0 because L % 32 == 0
+        const uint32_t tpc = 256u / (T * T / 2u); // tiles % tpc == 0 because L % 32 == 0
+        PdlLaunch pl(dim3(tiles / tpc), dim3(256), 64 + tpc * slab, st, pdl);
         if (g.kind == RNG_LFIB1279)
-            ising_multihit_kernel<RNG_LFIB1279, false><<<grid, 256, 64 + tpc * slab, st>>>(g, d_spins, L, tab, T, k_hits,
-                                                                                          (uint32_t)coarse, tiles);
+            e = cudaLaunchKernelEx(&pl.cfg, ising_multihit_kernel<RNG_LFIB1279, false>, g, d_spins, L, tab, T, k_hits, C, tiles);
         else
-            ising_multihit_kernel<RNG_LFIB521, false><<<grid, 256, 64 + tpc * slab, st>>>(g, d_spins, L, tab, T, k_hits,
-                                                                                         (uint32_t)coarse, tiles);
+            e = cudaLaunchKernelEx(&pl.cfg, ising_multihit_kernel<RNG_LFIB521, false>, g, d_spins, L, tab, T, k_hits, C, tiles);
     } else if (T == 8u) { // one warp per tile, four tiles per CTA
-        const uint32_t wpc = 4u, grid = (tiles + wpc - 1u) / wpc;
-#define MH(KIND)                                                                                                  \
-    ising_multihit_kernel<KIND, true><<<grid, wpc * 32u, 64 + wpc * slab, st>>>(g, d_spins, L, tab, T, k_hits, \
-                                                                                 (uint32_t)coarse, tiles)
+        const uint32_t wpc = 4u;
+        PdlLaunch pl(dim3((tiles + wpc - 1u) / wpc), dim3(wpc * 32u), 64 + wpc * slab, st, pdl);
+#define MH(KIND) e = cudaLaunchKernelEx(&pl.cfg, ising_multihit_kernel<KIND, true>, g, d_spins, L, tab, T, k_hits, C, tiles)
         RNGB200_DISPATCH_KIND(g.kind, MH)
 #undef MH
     } else {
-#define MH(KIND)                                                                                               \
-    ising_multihit_kernel<KIND, false><<<tiles, T * T / 2u, 64 + slab, st>>>(g, d_spins, L, tab, T, k_hits, \
-                                                                              (uint32_t)coarse, tiles)
+        PdlLaunch pl(dim3(tiles), dim3(T * T / 2u), 64 + slab, st, pdl);
+#define MH(KIND) e = cudaLaunchKernelEx(&pl.cfg, ising_multihit_kernel<KIND, false>, g, d_spins, L, tab, T, k_hits, C, tiles)
         RNGB200_DISPATCH_KIND(g.kind, MH)
 #undef MH
     }
     count_launch();
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 } // namespace rngb200
