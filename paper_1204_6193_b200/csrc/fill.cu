@@ -310,6 +310,7 @@ __global__ void __launch_bounds__(FILL_WARPS * 32) rowtile_fill_kernel(Gen g, ui
 template <bool F32>
 __global__ void __launch_bounds__(256) lcg_intra_fill_kernel(Gen g, uint32_t *__restrict__ out, uint64_t n)
 {
+    pdl_entry(); // back-to-back calls on one handle: the state comes from the previous launch (internal.h)
     const uint64_t s = blockIdx.x;
     const uint32_t t = threadIdx.x;
     const LcgTable *__restrict__ tab = g.lcg;
@@ -354,10 +355,13 @@ __global__ void __launch_bounds__(256) lcg_intra_fill_kernel(Gen g, uint32_t *__
 static cudaError_t launch_lcg_intra(const Gen &g, void *d_out, uint64_t n, bool f32, cudaStream_t st)
 {
     if (g.S > 0x7fffffffull) return cudaErrorInvalidConfiguration;
-    if (f32) lcg_intra_fill_kernel<true><<<(unsigned)g.S, 256, 0, st>>>(g, (uint32_t *)d_out, n);
-    else lcg_intra_fill_kernel<false><<<(unsigned)g.S, 256, 0, st>>>(g, (uint32_t *)d_out, n);
+    // small grids (this path is chosen for few streams) are launch-bound: programmatic dependent launch
+    PdlLaunch pl(dim3((unsigned)g.S), dim3(256), 0, st, g.S * 256ull <= kPdlMaxThreads);
+    uint32_t *o = (uint32_t *)d_out;
+    const cudaError_t e = f32 ? cudaLaunchKernelEx(&pl.cfg, lcg_intra_fill_kernel<true>, g, o, n)
+                              : cudaLaunchKernelEx(&pl.cfg, lcg_intra_fill_kernel<false>, g, o, n);
     count_launch();
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 static int g_sm_count = 0;
