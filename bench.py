@@ -432,7 +432,7 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
 
 # (name, steps, warmup): the secondary configs of --suite full; sized so that the whole
 # default run stays within a few minutes
-SUITE = [("C2_f32", 20, 3), ("C1_u32", 200, 10), ("C1_f32", 200, 10), ("C1big_u32", 20, 3), ("C3fill_u32", 20, 3),
+SUITE = [("C2_f32", 20, 3), ("C1_u32", 1000, 20), ("C1_f32", 1000, 20), ("C1big_u32", 20, 3), ("C3fill_u32", 20, 3),
          ("C3_draw", 20, 3), ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1),
          ("C5b_xorwow_K8", 1, 1),
          ("N1_philox7_u32", 20, 3), ("N1_lcg32_u32", 20, 3), ("N1_philox7_draw", 20, 3), ("N1_philox10_draw", 20, 3),
