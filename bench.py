@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the hot path on B200(s), one JSON line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--suite primary|full]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--suite primary|baseline|full]
     python bench.py --impl reference ...        # the CPU oracle on the host cores
 
 A "step" is one pass of the hot path over one batch of the named workload (seeded,
@@ -10,8 +10,12 @@ BASELINE.json's metric is quoted on, Philox4x32-10, 2^20 streams x 1024 u32 = 4 
 that is one rng_fill_u32 call.  `value` is whole-job throughput with the output
 resident in HBM; `e2e` is the same metric through the host-buffer C-ABI call
 (rng_fill_u32_host into pinned host memory, device->host copy inside the timed region).
-`--suite full` (default at N=1) also measures the other BASELINE configs (C1, C3, C4, C5b)
-and reports them under "configs" in the same line.  See DESIGN.md section 7.
+The stdout line is ONE compact JSON object (< 4 KB, tests/test_bench_contract.py).  `--suite
+baseline` (default at N=1 for the default workload) also measures BASELINE.json's other configs
+(C1, C2 f32, C3, C4, C5b) and adds them as `"configs"`: rows of [workload, value, unit,
+roofline frac]; `--suite full` measures every workload of the registry.  Per-workload detail goes
+to stderr (one short line each) and, with `--dump PATH`, as a JSON list to that file.
+`config.workload` is the same short name (`--workload`) in both arms.  See DESIGN.md section 7.
 """
 from __future__ import annotations
 
@@ -47,29 +51,44 @@ def measured_peaks() -> dict:
 N_SM, SMSP_PER_SM, LANES = 148, 4, 32  # B200: 148 SMs x 4 schedulers x 1 warp-instruction/clk
 
 
-def measured_traffic(name: str):
-    """DRAM bytes per launch of the workload's dominant kernel from the committed `ncu --set full`
-    capture (profiles/traffic.json, written from the raw page; never measured under this run)"""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
+
+
+def _capture(name: str):
+    """the workload's entry of profiles/traffic.json: figures of its dominant kernel from the committed
+    `ncu --set full` capture (written by `python -m paper_1204_6193_b200.ncu_summary` from ncu's raw page).
+    STATIC: captured in an earlier run of the same command under ncu, never measured in the run that prints it."""
     try:
-        return json.load(open(p)).get(name, {}).get("dram_bytes_per_launch")
+        return json.load(open(TRAFFIC_JSON)).get(name)
     except Exception:
         return None
+
+
+def measured_traffic(name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (static capture)"""
+    e = _capture(name)
+    return e.get("dram_bytes_per_launch") if e else None
+
+
+PIPES = ("alu", "fma", "fmaheavy", "lsu")
 
 
 def measured_ncu(name: str):
-    """ncu-measured utilisation of the workload's dominant kernel from the same committed capture: issue slots,
-    alu / fma / lsu pipes (pct of peak sustained), fma-heavy pipe cycles, DRAM throughput; None if not captured"""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
-    try:
-        e = json.load(open(p)).get(name)
-        if not e:
-            return None
-        keys = ("kernel", "ncu_time_us", "issue_active_pct", "pipe_alu_pct", "pipe_fma_pct",
-                "pipe_fmaheavy_cycles_pct_of_elapsed", "pipe_lsu_pct", "dram_throughput_pct", "source")
-        return {k: e.get(k) for k in keys}
-    except Exception:
+    """ncu-measured utilisation of the workload's dominant kernel (static capture): issue slots, the busiest
+    pipe and its utilisation, DRAM throughput; None if this workload was not captured"""
+    e = _capture(name)
+    if not e:
         return None
+    pipes = {"alu": e.get("pipe_alu_pct"), "fma": e.get("pipe_fma_pct"), "lsu": e.get("pipe_lsu_pct"),
+             "fmaheavy": e.get("pipe_fmaheavy_cycles_pct_of_elapsed")}
+    pipes = {k: v for k, v in pipes.items() if v is not None}
+    top = max(pipes, key=pipes.get) if pipes else None
+    r1 = lambda v: None if v is None else round(float(v), 1)  # noqa: E731
+    return {"issue_active_pct": r1(e.get("issue_active_pct")), "binding_pipe": top,
+            "binding_pipe_pct": r1(pipes.get(top)) if top else None,
+            "dram_throughput_pct": r1(e.get("dram_throughput_pct")), "time_us": e.get("ncu_time_us"),
+            "kernel": (e.get("kernel") or "").replace("void ", "").split("(")[0],
+            "capture": e.get("source"), "measured_in_this_run": False}
 
 
 def issue_peak_tinst(sm_mhz: float) -> float:
@@ -320,7 +339,37 @@ class IsingJob(Job):
         self.rng.close()
 
 
-def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, dev_index: int) -> dict:
+def roofline(name: str, bound: str, alg_per_launch: float, sec_per_launch: float, store_gbs=None) -> dict:
+    """the `roofline` object of one workload.  hbm: algorithmic bytes per launch / measured launch duration against
+    the measured copy bandwidth (MEASURED_PEAKS.json), and against the live write-only (memset) ceiling of this run
+    when it was probed (a fill only writes; a copy reads and writes).  alu: the ncu-measured issue-slot and
+    binding-pipe utilisation lead (static capture); achieved/peak/frac are the hand-counted algorithmic
+    thread-instructions against the issue-slot peak, tagged as such."""
+    peaks = measured_peaks()
+    ncu = measured_ncu(name)
+    if bound == "hbm":
+        ach = alg_per_launch / sec_per_launch / 1e9
+        r = {"bound": "hbm", "achieved": round(ach, 1), "peak": peaks["hbm_gbs"], "unit": "GB/s",
+             "frac": round(ach / peaks["hbm_gbs"], 4), "traffic": measured_traffic(name),
+             "algorithmic_bytes": int(alg_per_launch), "peak_source": peaks["source"] + " copy bandwidth"}
+        if store_gbs:
+            r["store_ceiling"] = round(store_gbs, 1)
+            r["frac_vs_store_ceiling"] = round(ach / store_gbs, 4)
+    else:
+        ach = alg_per_launch / sec_per_launch / 1e12
+        peak = issue_peak_tinst(peaks["sm_max_mhz"])
+        r = {"bound": "alu", "achieved": round(ach, 3), "peak": round(peak, 3), "unit": "Tinst/s",
+             "frac": round(ach / peak, 4), "basis": "algorithmic instruction count", "traffic": measured_traffic(name),
+             "peak_source": "148 SM x 4 SMSP x 32 lanes x sm_max_mhz issue slots"}
+        if ncu:
+            r["ncu_issue_active_pct"] = ncu["issue_active_pct"]
+            r["ncu_binding_pipe"] = f"{ncu['binding_pipe']} {ncu['binding_pipe_pct']}%"
+    r["ncu"] = ncu
+    return r
+
+
+def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, dev_index: int,
+            store_gbs=None) -> dict:
     """W untimed warm-up steps, then EXACTLY `steps` steps between barrier+synchronize,
     timed with CUDA events on the launching stream; max over ranks."""
     import torch
@@ -356,21 +405,8 @@ def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, 
     res = {"name": job.name, "value": value, "unit": job.unit, "steps": steps, "warmup": warmup,
            "ms_per_step": ms / steps, "gpu_launches": int(launches), "dtype": job.dtype}
     # roofline of the (single) dominant kernel: average launch duration = timed region / launches
-    peaks = measured_peaks()
     n_l = steps if isinstance(job, SeedJob) else max(int(launches), 1)  # SeedJob counts per step (many small launches)
-    sec_per_launch = ms * 1e-3 / n_l
-    if job.bound == "hbm":
-        ach = job.alg_per_launch() / sec_per_launch / 1e9
-        res["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                           "frac": ach / peaks["hbm_gbs"], "traffic": measured_traffic(job.name),
-                           "algorithmic_bytes": job.alg_per_launch(), "peak_source": peaks["source"] + " copy bandwidth"}
-    else:
-        ach = job.alg_per_launch() / sec_per_launch / 1e12
-        peak = issue_peak_tinst(peaks["sm_max_mhz"])
-        res["roofline"] = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tinst/s", "frac": ach / peak,
-                           "traffic": measured_traffic(job.name),
-                           "peak_source": "148 SM x 4 SMSP x 32 lanes x sm_max_mhz (issue slots; DESIGN.md s7)"}
-    res["roofline"]["ncu"] = measured_ncu(job.name)
+    res["roofline"] = roofline(job.name, job.bound, job.alg_per_launch(), ms * 1e-3 / n_l, store_gbs)
     if clocks:
         res["clocks"] = clocks
     if job.name in PAPER_GTX480:
@@ -447,11 +483,18 @@ SUITE = [("C2_f32", 20, 3), ("C1_u32", 1000, 20), ("C1_f32", 1000, 20), ("C1big_
 # ------------------------------------------------------------------------------------
 # the CPU oracle legs (the only places bench.py executes oracle/)
 # ------------------------------------------------------------------------------------
-def oracle_sample_rate(workload: str, target_s: float = 4.0) -> dict:
-    """time the oracle, as it stands, on a bounded sample of the workload on all host
-    cores; returns {"value","unit","cores","kind","sample","seconds"}"""
-    import numpy as np
+def oracle_sample_rate(workload: str, target_s: float = 4.0, threads: int | None = None) -> dict:
+    """time the oracle, as it stands, on a bounded sample of the workload on all host cores (or on `threads`
+    of them: the oracle's only concession to run time is `omp parallel for` over independent streams, and
+    orc_set_threads(1) turns that off); returns {"value","unit","cores","kind","sample","seconds"}"""
     import oracle
+    if threads is not None:
+        all_cores = oracle.threads()
+        oracle.set_threads(threads)
+        try:
+            return oracle_sample_rate(workload, target_s)
+        finally:
+            oracle.set_threads(all_cores)
     cores = oracle.threads()
     if workload.startswith("T1"):
         cfg = {"T1_xorwow_k1": W.T1_XORWOW_K1, "T1_xorwow_k100": W.T1_XORWOW_K100, "T1_philox_k100": W.T1_PHILOX_K100,
@@ -605,22 +648,63 @@ def run_e2e(job: Job, steps: int, warmup: int, world: int) -> dict:
     val = job.units_per_step() * steps * world / (ms * 1e-3) / 1e9
     return {"value": val, "unit": job.unit, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": steps,
             "ms_per_step": ms / steps, "api": api,
-            "note": "inputs of this path are scalars (kind, n_streams, seed): nothing but the result crosses the bus"
+            "note": "inputs are scalars (kind, n_streams, seed); the result crosses the bus every step"
             if h2d == 0 else "lattice copied host->device and back every step"}
+
+
+SHORT_DESC = {
+    "C2_u32": "Philox4x32-10, 2^20 streams x 1024 u32 = 4 GiB per step (BASELINE configs[1])",
+    "C2_f32": "Philox4x32-10, 2^20 streams x 1024 f32 = 4 GiB per step (BASELINE configs[1], float variant)",
+}
+
+# BASELINE.json's own configs besides the headline: (workload, steps, warmup) of --suite baseline
+BASELINE_SUITE = [("C2_f32", 20, 3), ("C1_u32", 1000, 20), ("C1_f32", 1000, 20), ("C3_draw", 20, 3),
+                  ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1)]
+
+
+def build_line(res: dict, args, world: int, cfg_info: dict, e2e=None, cpu=None, ceil=None, configs=None) -> dict:
+    """the ONE stdout JSON object of the b200 arm (kept compact: the driver reads the last few KB of stdout).
+    `res` is run_job()'s result for the headline workload, `configs` the other workloads' results."""
+    line = {
+        "metric": METRIC, "value": res["value"], "unit": res["unit"], "n_gpus": world, "steps": res["steps"],
+        "warmup": res["warmup"], "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None,  # BASELINE.md holds no published number for this metric on this workload
+        "dtype": res["dtype"], "data": "synthetic (seeded streams; this path has no dataset)", "impl": "b200",
+        "config": {"workload": args.workload, "name": res["name"], **cfg_info, "parallelism": f"streams x{world}"},
+        "clocks": res.get("clocks"), "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],
+    }
+    if "paper_gtx480" in res:
+        pg = res["paper_gtx480"]
+        line["paper_gtx480"] = {"value": pg["value"], "unit": pg["unit"], "cite": pg["cite"], "ratio": round(pg["ratio"], 1)}
+    if e2e:
+        line["e2e"] = e2e
+    if cpu:
+        line["cpu_baseline"] = cpu
+    if ceil:
+        line["hbm_ceilings_measured_live"] = {k: round(v, 1) for k, v in ceil.items()}
+    # only BASELINE.json's own configs ride on the line; --suite full's other workloads go to stderr / --dump
+    own = {n for n, _, _ in BASELINE_SUITE}
+    rows = [[c["workload"], round(c["value"], 2), c["unit"], c["roofline"]["bound"], c["roofline"]["frac"]]
+            for c in (configs or []) if c["workload"] in own]
+    if rows:
+        line["configs_cols"] = ["workload", "value", "unit", "roofline_bound", "roofline_frac"]
+        line["configs"] = rows
+    return line
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C2_u32")
-    ap.add_argument("--suite", default=None, choices=["primary", "full"])
+    ap.add_argument("--suite", default=None, choices=["primary", "baseline", "full"])
     ap.add_argument("--ising-sweeps", type=int, default=1000, help="sweeps per Ising step (config: 1000)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dump", default=None, help="also write every workload's full result as a JSON list to this file")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         log("[bench] note: timing rules ask for >= 3 warm-up steps")
@@ -645,52 +729,50 @@ def main():
         torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         torch.distributed.barrier()
     pkg.lib()
-    suite = args.suite or ("full" if world == 1 and args.workload == "C2_u32" else "primary")
+    suite = args.suite or ("baseline" if world == 1 and args.workload == "C2_u32" else "primary")
     buf = torch.empty(1 << 30, dtype=torch.int32, device="cuda")  # 4 GiB, reused by every workload (> L2)
 
+    # write-only and copy ceilings of this box, measured before the timed region with library calls
+    ceil = hbm_ceilings(buf)
+    store_gbs = ceil["memset_write_gbs"]
+
     job = make_job(args.workload, rank, world, buf, args.ising_sweeps)
-    res = run_job(job, args.steps, args.warmup, world, sample_clocks=True, dev_index=local_rank)
+    res = run_job(job, args.steps, args.warmup, world, sample_clocks=True, dev_index=local_rank, store_gbs=store_gbs)
     e2e = None if args.no_e2e else run_e2e(job, args.e2e_steps, 1, world)
+    cfg_info = {"desc": SHORT_DESC.get(args.workload, res["name"]),
+                "streams_per_gpu": getattr(getattr(job, "cfg", None), "n_streams", getattr(job, "n_local", None)),
+                "l2": "64 MiB lattice is L2-resident by design (DESIGN.md s7)" if isinstance(job, IsingJob)
+                else "4 GiB output per step > 126 MB L2, no flush needed"}
     job.close()
-    ceil = hbm_ceilings(buf) if rank == 0 and world == 1 else None
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = oracle_sample_rate(args.workload, 4.0)
-        cpu.pop("seconds", None)
+        cpu = oracle_sample_rate(args.workload, 8.0)
+        cpu["seconds"] = round(cpu["seconds"], 2)
+        one = oracle_sample_rate(args.workload, 6.0, threads=1)
+        cpu["single_thread"] = {"value": one["value"], "unit": one["unit"], "cores": 1, "sample": one["sample"],
+                                "seconds": round(one["seconds"], 2)}
 
     configs = []
-    if suite == "full":
-        for name, k, w in SUITE:
-            if name == args.workload:
-                continue
-            j = make_job(name, rank, world, buf, args.ising_sweeps)
-            r = run_job(j, k, w, world, sample_clocks=False, dev_index=local_rank)
-            j.close()
-            configs.append(r)
-            log(f"[bench] {r['name']}: {r['value']:.2f} {r['unit']}  {r['ms_per_step']:.3f} ms/step  "
-                f"roofline {r['roofline']['bound']} {r['roofline']['frac']:.3f}")
+    todo = BASELINE_SUITE if suite == "baseline" else SUITE if suite == "full" else []
+    for name, k, w in todo:
+        if name == args.workload:
+            continue
+        j = make_job(name, rank, world, buf, args.ising_sweeps)
+        r = run_job(j, k, w, world, sample_clocks=False, dev_index=local_rank, store_gbs=store_gbs)
+        j.close()
+        r["workload"] = name
+        configs.append(r)
+        rl = r["roofline"]
+        extra = f" (vs store ceiling {rl['frac_vs_store_ceiling']:.3f})" if "frac_vs_store_ceiling" in rl else \
+            f" (ncu issue {rl.get('ncu_issue_active_pct')}%, {rl.get('ncu_binding_pipe')})" if rl["bound"] == "alu" else ""
+        log(f"[bench] {name} = {r['name']}: {r['value']:.2f} {r['unit']}  {r['ms_per_step']:.3f} ms/step  "
+            f"roofline {rl['bound']} {rl['frac']:.3f}{extra}")
 
     if rank == 0:
-        line = {
-            "metric": METRIC, "value": res["value"], "unit": res["unit"], "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": res["paper_gtx480"]["ratio"] if "paper_gtx480" in res else None, "dtype": res["dtype"],
-            "data": "synthetic (seeded streams; this path has no dataset)",
-            "config": {"workload": res["name"], "l2": "4 GiB output per step, larger than the 126 MB L2"
-                       if not isinstance(job, IsingJob) else "64 MiB lattice is L2-resident by design (DESIGN.md s7)",
-                       "streams_per_gpu": getattr(getattr(job, "cfg", None), "n_streams", getattr(job, "n_local", None)), "parallelism": f"streams x{world}"},
-            "clocks": res.get("clocks"), "gpu_launches": res["gpu_launches"], "roofline": res["roofline"],
-        }
-        if "paper_gtx480" in res:
-            line["paper_gtx480"] = res["paper_gtx480"]
-        if e2e:
-            line["e2e"] = e2e
-        if cpu:
-            line["cpu_baseline"] = cpu
-        if ceil:
-            line["hbm_ceilings_measured_live"] = ceil
-        if configs:
-            line["configs"] = configs
+        line = build_line(res, args, world, cfg_info, e2e, cpu, ceil if world == 1 else None, configs)
+        if args.dump:
+            with open(args.dump, "w") as f:
+                json.dump([dict(res, workload=args.workload)] + configs, f, indent=1)
         print(json.dumps(line), flush=True)
     if world > 1:
         torch.distributed.barrier()
