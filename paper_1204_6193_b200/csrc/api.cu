@@ -56,7 +56,52 @@ int ensure_staging(rng_handle *h, uint64_t bytes)
 
 namespace rngb200 {
 void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+int sm_count(int device)
+{
+    static std::atomic<int> cache[64];
+    if (device < 0 || device >= 64) return 148;
+    int v = cache[device].load(std::memory_order_relaxed);
+    if (v <= 0) {
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || v <= 0) {
+            cudaGetLastError();
+            v = 148;
+        }
+        cache[device].store(v, std::memory_order_relaxed);
+    }
+    return v;
+}
 } // namespace rngb200
+
+namespace {
+// a handle's buffers live on the device that was current at rng_create: every entry point that launches on them
+// must be called with that device current (launch configuration and function attributes are per device too)
+int check_device(const rng_handle *h, const char *name)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(RNG_E_CUDA, "%s: no current CUDA device", name);
+    }
+    if (dev != h->device)
+        return fail(RNG_E_INVAL, "%s: handle was created on device %d but device %d is current", name, h->device, dev);
+    return RNG_OK;
+}
+#define CHECK_DEVICE(h, name)                  \
+    do {                                       \
+        int rc__ = check_device((h), (name));  \
+        if (rc__) return rc__;                 \
+    } while (0)
+// a launch inside a multi-launch call failed: the launches before it are enqueued and will advance the generator
+// state, so the handle's draw counter must say so before the error is returned
+#define CU_AT(call, h, d)                               \
+    do {                                                \
+        cudaError_t e__ = (call);                       \
+        if (e__ != cudaSuccess) {                       \
+            (h)->g.draws_done = (d);                    \
+            return cuda_fail(e__, #call);               \
+        }                                               \
+    } while (0)
+} // namespace
 
 extern "C" {
 
@@ -122,7 +167,12 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
     if (e == cudaSuccess && (kind == RNG_LCG64 || kind == RNG_LCG64_LEAPFROG || kind == RNG_LCG32_LEAPFROG))
         e = cudaMalloc(&tab, sizeof(LcgTable));
     h->g.lcg = tab;
-    if (e == cudaSuccess) e = cudaMalloc(&h->energy_scratch, sizeof(int64_t));
+    if (e == cudaSuccess) e = cudaMalloc(&h->energy_scratch, 2 * sizeof(int64_t));
+    if (e == cudaSuccess) {
+        h->ticket = (uint64_t *)(h->energy_scratch + 1);
+        h->ticket_base = 0;
+        e = cudaMemsetAsync(h->ticket, 0, sizeof(uint64_t), 0);
+    }
     if (e == cudaSuccess)
         e = (kind == RNG_XS1024W_SKIP)                       ? launch_seed_xs1024_skip(h->g, 0)
             : (kind == RNG_LFIB521 || kind == RNG_LFIB1279) ? launch_seed_lfib(h->g, 0)
@@ -163,6 +213,7 @@ static int fill_common(rng_handle *h, void *d_out, uint64_t n, bool f32, void *s
     if (!aligned(d_out, 16)) return fail(RNG_E_INVAL, "%s: d_out must be 16-byte aligned", name);
     if (mul_overflows(h->g.S, n) || h->g.S * n > (1ull << 60)) return fail(RNG_E_INVAL, "%s: n_streams*n too large", name);
     if (h->g.draws_done + n < n) return fail(RNG_E_INVAL, "%s: draw counter would overflow", name);
+    CHECK_DEVICE(h, name);
     CU(launch_fill(*h, d_out, n, f32, (cudaStream_t)stream));
     h->g.draws_done += n;
     return RNG_OK;
@@ -183,6 +234,7 @@ int rng_draw_reduce(rng_handle *h, uint32_t *d_out, uint64_t n, void *stream)
     if (!d_out) return fail(RNG_E_INVAL, "rng_draw_reduce: d_out is NULL");
     if (!aligned(d_out, 8)) return fail(RNG_E_INVAL, "rng_draw_reduce: d_out must be 8-byte aligned");
     if (h->g.draws_done + n < n) return fail(RNG_E_INVAL, "rng_draw_reduce: draw counter would overflow");
+    CHECK_DEVICE(h, "rng_draw_reduce");
     CU(launch_draw_reduce(*h, d_out, n, (cudaStream_t)stream));
     h->g.draws_done += n;
     return RNG_OK;
@@ -214,6 +266,7 @@ int ising_sweep(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_
     const uint64_t K = half / h->g.S;
     if (mul_overflows(2 * K, n_sweeps) || h->g.draws_done + 2 * K * n_sweeps < h->g.draws_done)
         return fail(RNG_E_INVAL, "ising_sweep: draw counter would overflow");
+    CHECK_DEVICE(h, "ising_sweep");
     IsingTable tab;
     ising_accept_table(beta, nullptr, tab.T);
     cudaStream_t st = (cudaStream_t)stream;
@@ -235,21 +288,21 @@ int ising_sweep(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_
         CU(launch_ising_ms_pack(d_spins, h->ms_planes, L, st));
         for (uint32_t t = 0; t < n_sweeps; t++) {
             for (int c = 0; c < 2; c++) {
-                CU(launch_ising_ms_half_sweep(*h, h->ms_planes, L, tab, K, d, c, st));
+                CU_AT(launch_ising_ms_half_sweep(*h, h->ms_planes, L, tab, K, d, c, st), h, d);
                 d += K;
             }
-            if (d_trace) CU(launch_ising_ms_energy(h->ms_planes, L, d_trace + t, st));
+            if (d_trace) CU_AT(launch_ising_ms_energy(h->ms_planes, L, d_trace + t, st), h, d);
         }
-        CU(launch_ising_ms_unpack(d_spins, h->ms_planes, L, st));
+        CU_AT(launch_ising_ms_unpack(d_spins, h->ms_planes, L, st), h, d);
         h->g.draws_done = d;
         return RNG_OK;
     }
     for (uint32_t t = 0; t < n_sweeps; t++) {
         for (int c = 0; c < 2; c++) {
-            CU(launch_ising_half_sweep(*h, d_spins, L, tab, K, d, c, st));
+            CU_AT(launch_ising_half_sweep(*h, d_spins, L, tab, K, d, c, st), h, d);
             d += K;
         }
-        if (d_trace) CU(launch_ising_energy(d_spins, L, d_trace + t, st));
+        if (d_trace) CU_AT(launch_ising_energy(d_spins, L, d_trace + t, st), h, d);
     }
     h->g.draws_done = d;
     return RNG_OK;
@@ -273,16 +326,17 @@ int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta
     const uint64_t per_sweep = 4ull * k_hits;
     if (mul_overflows(per_sweep, n_sweeps) || h->g.draws_done + per_sweep * n_sweeps < h->g.draws_done)
         return fail(RNG_E_INVAL, "ising_sweep_multihit: draw counter would overflow");
+    CHECK_DEVICE(h, "ising_sweep_multihit");
     IsingTable tab;
     ising_accept_table(beta, nullptr, tab.T);
     cudaStream_t st = (cudaStream_t)stream;
     uint64_t d = h->g.draws_done;
     for (uint32_t t = 0; t < n_sweeps; t++) {
         for (int c = 0; c < 2; c++) {
-            CU(launch_ising_multihit(*h, d_spins, L, tab, tile, k_hits, d, c, st));
+            CU_AT(launch_ising_multihit(*h, d_spins, L, tab, tile, k_hits, d, c, st), h, d);
             d += 2ull * k_hits;
         }
-        if (d_trace) CU(launch_ising_energy(d_spins, L, d_trace + t, st));
+        if (d_trace) CU_AT(launch_ising_energy(d_spins, L, d_trace + t, st), h, d);
     }
     h->g.draws_done = d;
     return RNG_OK;
@@ -310,6 +364,7 @@ static int fill_host_common(rng_handle *h, void *h_out, uint64_t n, bool f32, vo
     if (!h_out) return fail(RNG_E_INVAL, "%s: h_out is NULL", name);
     if (mul_overflows(h->g.S, n) || h->g.S * n > (1ull << 58)) return fail(RNG_E_INVAL, "%s: n_streams*n too large", name);
     const uint64_t bytes = h->g.S * n * 4;
+    CHECK_DEVICE(h, name);
     int rc = ensure_staging(h, bytes);
     if (rc) return rc;
     rc = fill_common(h, h->staging, n, f32, stream, name);
@@ -330,6 +385,7 @@ int rng_draw_reduce_host(rng_handle *h, uint32_t *h_out, uint64_t n, void *strea
 {
     if (!h || !h_out) return fail(RNG_E_INVAL, "rng_draw_reduce_host: NULL argument");
     const uint64_t bytes = h->g.S * 8;
+    CHECK_DEVICE(h, "rng_draw_reduce_host");
     int rc = ensure_staging(h, bytes);
     if (rc) return rc;
     rc = rng_draw_reduce(h, (uint32_t *)h->staging, n, stream);
@@ -345,6 +401,7 @@ int ising_sweep_host(rng_handle *h, int8_t *h_spins, uint32_t L, double beta, ui
     if (L < 4 || (L & 1u)) return fail(RNG_E_INVAL, "ising_sweep_host: L must be even and >= 4");
     const uint64_t N = (uint64_t)L * L;
     const uint64_t sp_bytes = (N + 15) & ~15ull, tr_bytes = h_trace ? 8ull * n_sweeps : 0;
+    CHECK_DEVICE(h, "ising_sweep_host");
     int rc = ensure_staging(h, sp_bytes + tr_bytes);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
@@ -374,6 +431,7 @@ int rng_get_state(rng_handle *h, void *h_buf, uint64_t bytes)
     if (bytes != h->state_bytes) return fail(RNG_E_INVAL, "rng_get_state: expected %llu bytes", (unsigned long long)h->state_bytes);
     if (!bytes) return RNG_OK;
     if (!h_buf) return fail(RNG_E_INVAL, "rng_get_state: h_buf is NULL");
+    CHECK_DEVICE(h, "rng_get_state");
     CU(cudaDeviceSynchronize());
     const int wps = h->g.kind == RNG_XORWOW ? 6 : h->g.kind == RNG_MWC_MULTI ? 3 : 0; // words per stream of the SoA kinds
     if (wps) { // device layout w[k*S+s] -> canonical [s][k]
@@ -394,6 +452,7 @@ int rng_set_state(rng_handle *h, const void *h_buf, uint64_t bytes)
     if (bytes != h->state_bytes) return fail(RNG_E_INVAL, "rng_set_state: expected %llu bytes", (unsigned long long)h->state_bytes);
     if (!bytes) return RNG_OK;
     if (!h_buf) return fail(RNG_E_INVAL, "rng_set_state: h_buf is NULL");
+    CHECK_DEVICE(h, "rng_set_state");
     CU(cudaDeviceSynchronize());
     const int wps = h->g.kind == RNG_XORWOW ? 6 : h->g.kind == RNG_MWC_MULTI ? 3 : 0;
     if (wps) {
@@ -415,6 +474,7 @@ int rng_set_variant(rng_handle *h, const char *name, int value)
     else if (!strcmp(name, "ising")) h->var_ising = value;
     else if (!strcmp(name, "store")) h->var_store = value;
     else if (!strcmp(name, "lcg")) h->var_lcg = value;
+    else if (!strcmp(name, "xsfill")) h->var_xsfill = value;
     else return fail(RNG_E_INVAL, "rng_set_variant: unknown name '%s'", name);
     return RNG_OK;
 }

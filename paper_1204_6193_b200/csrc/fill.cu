@@ -70,7 +70,11 @@ __global__ void __launch_bounds__(256) philox_fill_kernel(uint32_t *__restrict__
 //  * U independent blocks per lane are interleaved (the full-tile path has no per-block
 //    predicate, so ptxas keeps them interleaved) and hide the IMAD -> LOP3 -> IMAD chain.
 //  * Persistent grid: warps stride over tiles; (row, tile-in-row) advance incrementally
-//    (one 64-bit division per warp).
+//    (one 64-bit division per warp).  Tried in round 2 and rejected: handing out chunks of tiles through an
+//    atomic ticket counter, which lifts the store-bound xs1024 fill (fill_xs1024.cu).  Here it measured
+//    651 us (static) against 673 us (tickets of 16 tiles) and 708 us (8 tiles) per 4 GiB: this kernel is bound by
+//    its IMAD.WIDE arithmetic, not by an uneven share of the write bandwidth, and same-address atomics cost
+//    about 3 ns each.
 // ------------------------------------------------------------------------------------
 // U independent 4-word blocks per lane (blocks rb0, rb0+32, ...), ten rounds interleaved,
 // one 128-bit streaming store each.  CHECK = bounds-check each block (ragged last tile).
@@ -364,16 +368,11 @@ static cudaError_t launch_lcg_intra(const Gen &g, void *d_out, uint64_t n, bool 
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-static int g_sm_count = 0;
 static int sm_count()
 {
-    if (!g_sm_count) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev);
-        if (g_sm_count <= 0) g_sm_count = 148;
-    }
-    return g_sm_count;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) cudaGetLastError();
+    return sm_count(dev);
 }
 
 template <int KIND>
@@ -403,7 +402,7 @@ static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uin
     const uint64_t tpr = (blocks_per_row + 32 * U * T - 1) / (32 * U * T);
     const uint64_t n_tiles = g.S * tpr;
     // persistent grid: a multiple of the SM count; 8 warps per CTA, CTAs resident per SM by registers
-    static int per_sm = 0;
+    static int per_sm = 0; // a property of the kernel on sm_100a; the same on every device this library targets
     if (!per_sm) {
         int b = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, philox_fill_warp_kernel<F32, U, T, R>, 256, 0);

@@ -160,6 +160,113 @@ __global__ void __launch_bounds__(WARPS * 32)
     if (TMA && pending && lane == 0) bulk_wait_read_all(); // the tile must outlive the copy that reads it
 }
 
+// ---- the fill kernel of the TMA path: persistent warps that draw their work from a ticket counter ----
+// One CTA per SM for the whole call; a warp processes items (an item = the K instances = 32K rows that one warp
+// hosts) until the tickets run out.  What this buys over one short-lived CTA per item (xs1024_fill_kernel<.., TMA =
+// true>, kept for comparison as variant "xsfill" 1):
+//   * the next item's state (K words per lane) is loaded while the current item is generated, so no warp sits on a
+//     global-load latency while holding 16 KiB of shared memory;
+//   * with NT = 2 tiles per warp the TMA unit reads tile A while the warp generates into tile B
+//     (cp.async.bulk.wait_group.read NT-1 before a tile is reused);
+//   * there is no CTA tail waiting for its last copy per item, only one per call.
+// With n = 64 per call (C4: 64 calls of 64 draws, the 4 GiB buffer holds no more) an item is just two tiles, so
+// these per-item costs were a large share of a warp's life.
+// Work distribution is DYNAMIC (atomic ticket per item, fetched one item ahead so that its latency and the state
+// load hide behind the generation): at the HBM limit the SMs of a B200 do not all get the same share of the write
+// bandwidth, and a static "item += number of warps" split waits for the slowest SM -- the bare store pattern of
+// this kernel runs at 5.9 TB/s with the static split and at 7.0-7.3 TB/s with tickets, which is what a grid of
+// one-shot CTAs gets from the hardware's own CTA scheduler (B200 microbenchmark).
+// Tickets: *ticket counts up for the life of the handle; this launch owns [base, base + n_items) and every warp
+// takes exactly one ticket beyond that range before it leaves, so the host knows the next launch's base.
+template <int K, bool F32, int WARPS, int NT>
+__global__ void __launch_bounds__(WARPS * 32, 1)
+    xs1024_fill_persistent_kernel(Gen g, uint64_t n, const __grid_constant__ CUtensorMap tmap,
+                                  unsigned long long *__restrict__ ticket, unsigned long long base)
+{
+    extern __shared__ uint32_t xs_tiles_raw[];
+    constexpr int P = 32 / K;
+    constexpr int ROWS = 32 * K;
+    constexpr uint32_t TILE_WORDS = ROWS * 32;
+    // SWIZZLE_128B wants the box 1 KiB aligned in shared memory (an offset into the array, so that the pointer
+    // keeps its address space and the tile stores stay STS)
+    const uint32_t pad = (1024u - ((uint32_t)__cvta_generic_to_shared(xs_tiles_raw) & 1023u)) & 1023u;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *tiles = xs_tiles_raw + (pad >> 2) + (uint32_t)warp * (NT * TILE_WORDS);
+    const uint64_t n_items = (g.S + ROWS - 1) / ROWS;
+    const int p = (P == 1) ? 0 : (lane & (P - 1));
+    uint32_t *state = (uint32_t *)g.state;
+    XsMasks<K> m;
+    m.init(p);
+    const uint32_t swz = (uint32_t)lane & 7u;
+    const uint32_t nupd0 = (uint32_t)g.draws_done;
+    uint32_t tcount = 0; // tiles handed to the TMA unit so far (all by lane 0 of this warp)
+
+    // One ticket per item: handing out chunks of 2..16 consecutive items per ticket measured 4-15 % SLOWER (the
+    // items being written at any moment then spread over a proportionally wider address window).
+    auto take = [&]() -> uint64_t { // warp-uniform next item
+        unsigned long long v = 0ull;
+        if (lane == 0) v = atomicAdd(ticket, 1ull) - base;
+        return __shfl_sync(0xffffffffu, v, 0);
+    };
+    uint32_t w[K], wn[K];
+    uint64_t item = take();
+    if (item >= n_items) return;
+    {
+        const uint64_t my0 = item * ROWS + (uint64_t)K * lane;
+#pragma unroll
+        for (int j = 0; j < K; j++) wn[j] = 0u;
+        if (my0 < g.S) load_words<K>(state + my0, wn);
+    }
+    while (item < n_items) {
+        const uint64_t my0 = item * ROWS + (uint64_t)K * lane;
+        const bool live = my0 < g.S;
+#pragma unroll
+        for (int j = 0; j < K; j++) w[j] = wn[j];
+        const uint64_t next = take();
+        { // prefetch the next item's state
+            const uint64_t nx = next * ROWS + (uint64_t)K * lane;
+#pragma unroll
+            for (int j = 0; j < K; j++) wn[j] = 0u;
+            if (next < n_items && nx < g.S) load_words<K>(state + nx, wn);
+        }
+        uint32_t nupd = nupd0;
+        for (uint64_t j0 = 0; j0 < n; j0 += 32) {
+            const uint32_t kk = (uint32_t)((n - j0 < 32ull) ? (n - j0) : 32ull); // a multiple of 4 (n % 4 == 0)
+            uint32_t *tile = tiles + (NT == 1 ? 0u : (tcount % NT) * TILE_WORDS);
+            uint32_t *myrows = tile + lane * 32;
+            for (uint32_t c = 0; 4u * c < kk; c++) {
+                uint32_t o[K][4];
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    xs1024_update_k<K>(w, m);
+                    nupd++;
+                    const uint32_t wt = xs1024_weyl_term(nupd);
+#pragma unroll
+                    for (int j = 0; j < K; j++) o[j][u] = out_word(wt + w[j], F32);
+                }
+                if (c == 0 && tcount >= NT) { // the copy that last read this tile must be done reading it
+                    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(NT - 1) : "memory");
+                    __syncwarp();
+                }
+                const uint32_t phys = (c ^ swz) * 4u;
+#pragma unroll
+                for (int j = 0; j < K; j++)
+                    *reinterpret_cast<uint4 *>(myrows + j * 1024 + phys) = make_uint4(o[j][0], o[j][1], o[j][2], o[j][3]);
+            }
+            fence_generic_to_async(); // my generic-proxy writes -> visible to the async proxy
+            __syncwarp();
+            if (lane == 0) {
+                tma_store_3d(&tmap, tile, (int)j0, (int)(item * 32ull), 0);
+                bulk_commit();
+            }
+            tcount++;
+        }
+        if (live) store_words<K>(state + my0, w);
+        item = next;
+    }
+    if (lane == 0) bulk_wait_read_all(); // the tiles must outlive the copies that read them
+}
+
 // In-register draw mode (row a6): {xor, sum} of n draws per stream.  The Weyl term is the
 // same for every word, so its sum is accumulated once per update and added at the end.
 template <int K, int THREADS>
@@ -246,15 +353,12 @@ static cudaError_t launch_xs_fill(const Gen &g, uint32_t *o, uint64_t n, bool f3
     constexpr size_t smem = (size_t)WARPS * 32 * K * 32 * 4;
     const uint64_t inst = g.S / 32, warps = (inst + K - 1) / K, grid = (warps + WARPS - 1) / WARPS;
     if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
-    static bool attr_set = false;
-    if (!attr_set && smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(xs1024_fill_kernel<K, true, WARPS, TMA>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(xs1024_fill_kernel<K, false, WARPS, TMA>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (smem > 48 * 1024) { // per device and cheap: set on every launch rather than behind a per-process flag
+        const cudaError_t e = f32 ? cudaFuncSetAttribute(xs1024_fill_kernel<K, true, WARPS, TMA>,
+                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                                  : cudaFuncSetAttribute(xs1024_fill_kernel<K, false, WARPS, TMA>,
+                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     if (f32) xs1024_fill_kernel<K, true, WARPS, TMA><<<(unsigned)grid, WARPS * 32, smem, st>>>(g, o, n, tm);
     else xs1024_fill_kernel<K, false, WARPS, TMA><<<(unsigned)grid, WARPS * 32, smem, st>>>(g, o, n, tm);
@@ -262,7 +366,38 @@ static cudaError_t launch_xs_fill(const Gen &g, uint32_t *o, uint64_t n, bool f3
     return cudaGetLastError();
 }
 
-// variant "xs1024" = K (0: default); variant "store": 0 = default, 1 = LDS/STG write-out, 2 = TMA tensor store
+template <int K, int WARPS, int NT>
+static cudaError_t launch_xs_fill_persistent(const rng_handle &h, uint64_t n, bool f32, const CUtensorMap &tm, int sms,
+                                             cudaStream_t st)
+{
+    const Gen &g = h.g;
+    constexpr size_t smem = (size_t)WARPS * NT * 32 * K * 32 * 4 + 1024; // + alignment slack
+    static_assert(smem <= 227 * 1024, "tiles exceed the shared memory of a CTA");
+    const uint64_t items = (g.S + 32 * K - 1) / (32 * K);
+    uint64_t grid = (items + WARPS - 1) / WARPS;
+    if (grid > (uint64_t)sms) grid = (uint64_t)sms;
+    auto kf = xs1024_fill_persistent_kernel<K, true, WARPS, NT>;
+    auto ku = xs1024_fill_persistent_kernel<K, false, WARPS, NT>;
+    // unconditional (cheap; a per-process flag would be wrong with more than one device)
+    cudaError_t e = cudaFuncSetAttribute(f32 ? kf : ku, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    unsigned long long *tk = (unsigned long long *)h.ticket;
+    if (f32) kf<<<(unsigned)grid, WARPS * 32, smem, st>>>(g, n, tm, tk, h.ticket_base);
+    else ku<<<(unsigned)grid, WARPS * 32, smem, st>>>(g, n, tm, tk, h.ticket_base);
+    count_launch();
+    e = cudaGetLastError();
+    if (e == cudaSuccess) h.ticket_base += items + grid * WARPS; // every warp takes one ticket past the range
+    return e;
+}
+
+// variant "xs1024" = K (0: default); variant "store": 0 = default, 1 = LDS/STG write-out, 2 = TMA tensor store;
+// variant "xsfill" (TMA path only): 0 = by row length (below), 1 = one short-lived warp per item (round 1's
+// kernel), 2 = persistent warps with one tile each, 3 = persistent warps with two ping-pong tiles each.
+// Default by row length n, from 4 GiB fills on a B200 (K = 4; TB/s for variants 1 / 2 / 3):
+//   n = 64: 5.70 / 6.16 / 4.00    n = 128: 5.52 / 6.02 / 3.99    n = 256: 5.04 / 4.85 / 4.29
+//   n = 1024: 4.70 / 4.28 / 4.64  n = 4096: 3.47 / 3.36 / 4.83
+// (short rows: the tiles of a warp complete whole rows at once and more warps matter; long rows: the next 128
+// bytes of a row should follow quickly, which the second tile does)
 cudaError_t launch_xs1024_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st)
 {
     uint32_t *o = (uint32_t *)d_out;
@@ -270,6 +405,23 @@ cudaError_t launch_xs1024_fill(const rng_handle &h, void *d_out, uint64_t n, boo
     alignas(64) CUtensorMap tm;
     memset(&tm, 0, sizeof tm);
     const bool tma = h.var_store != 1 && make_out_tensor_map(&tm, o, h.g.S, n, K);
+    const int mode = h.var_xsfill >= 1 && h.var_xsfill <= 3 ? h.var_xsfill : n <= 128 ? 2 : n < 2048 ? 1 : 3;
+    if (tma && mode != 1) {
+        const int sms = sm_count(h.device);
+        const bool pp = mode == 3;
+        // warps per CTA = what 224 KiB of tiles allow
+        switch (K) {
+        case 1: return pp ? launch_xs_fill_persistent<1, 28, 2>(h, n, f32, tm, sms, st)
+                          : launch_xs_fill_persistent<1, 32, 1>(h, n, f32, tm, sms, st);
+        case 2: return pp ? launch_xs_fill_persistent<2, 14, 2>(h, n, f32, tm, sms, st)
+                          : launch_xs_fill_persistent<2, 28, 1>(h, n, f32, tm, sms, st);
+        case 8: return pp ? launch_xs_fill_persistent<8, 3, 2>(h, n, f32, tm, sms, st)
+                          : launch_xs_fill_persistent<8, 7, 1>(h, n, f32, tm, sms, st);
+        case 16: return launch_xs_fill_persistent<16, 3, 1>(h, n, f32, tm, sms, st);
+        default: return pp ? launch_xs_fill_persistent<4, 7, 2>(h, n, f32, tm, sms, st)
+                           : launch_xs_fill_persistent<4, 14, 1>(h, n, f32, tm, sms, st);
+        }
+    }
 #define XSF(KK, WARPS) \
     (tma ? launch_xs_fill<KK, WARPS, true>(h.g, o, n, f32, tm, st) : launch_xs_fill<KK, WARPS, false>(h.g, o, n, f32, tm, st))
     switch (K) {

@@ -50,9 +50,13 @@ struct rng_handle {
     void *staging;          // device staging for the *_host entry points
     uint64_t staging_bytes;
     int64_t *energy_scratch; // device, 1 x int64
+    // work tickets of the persistent fill kernels: a device counter that only counts up; a launch owns
+    // [ticket_base, ticket_base + its number of work items) and the host adds what the launch consumes
+    uint64_t *ticket;            // device, 1 x uint64 (zero at rng_create)
+    mutable uint64_t ticket_base;
     uint32_t *ms_planes;     // device scratch of the multi-spin Ising path: two bit planes of L*L/64 words
     uint64_t ms_planes_bytes;
-    int var_xs1024, var_ising, var_store, var_lcg;
+    int var_xs1024, var_ising, var_store, var_lcg, var_xsfill;
     int api_kind; // the kind rng_create was called with (g.kind is RNG_XS1024W for RNG_XS1024W_SKIP)
 };
 
@@ -109,6 +113,8 @@ __device__ __forceinline__ void pdl_entry()
 #endif
 
 void count_launch(uint64_t n = 1);
+// number of SMs of `device` (cached per device; 148 on a B200)
+int sm_count(int device);
 
 // seed.cu
 cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st);

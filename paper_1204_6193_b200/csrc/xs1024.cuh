@@ -25,9 +25,14 @@ namespace rngb200 {
 // from one of two lanes, D = 10/K or D+1 lanes away (K = 32: none).  A mask is all-ones when
 // that lane belongs to the instance; it is made opaque to the compiler so that it stays an
 // AND operand that folds into the LOP3 of the xor (instead of one SEL per shuffled word).
+// A word whose two sources sit in DIFFERENT lanes (D and D+1 away; one such word per phase, every word for K = 1)
+// is masked AFTER the funnel shift: the shifted word takes its upper bits from one source and its lower bits
+// from the other, so "source a masked by ma, source b by mb" equals the shift of the unmasked pair ANDed with
+// the same shift of (ma, mb) -- a per-lane constant per phase (mix[]), which again folds into the xor's LOP3.
 template <int K>
 struct XsMasks {
     uint32_t down[2], up[2]; // [0]: D lanes away, [1]: D+1 lanes away
+    uint32_t mix[3];         // phases A, B, C: the shifted pair of masks for a word with sources in both lanes
     __device__ __forceinline__ void init(int p)
     {
         constexpr int P = 32 / K, D = 10 / K;
@@ -35,16 +40,24 @@ struct XsMasks {
         for (int i = 0; i < 2; i++) {
             down[i] = (p + D + i < P) ? 0xffffffffu : 0u;
             up[i] = (p >= D + i) ? 0xffffffffu : 0u;
-            if (P > 1) {
+        }
+        mix[0] = __funnelshift_l(down[1], down[0], 9);
+        mix[1] = __funnelshift_r(up[0], up[1], 27);
+        mix[2] = __funnelshift_l(down[1], down[0], 24);
+        if (P > 1) {
+#pragma unroll
+            for (int i = 0; i < 2; i++) {
                 asm volatile("" : "+r"(down[i]));
                 asm volatile("" : "+r"(up[i]));
             }
+#pragma unroll
+            for (int i = 0; i < 3; i++) asm volatile("" : "+r"(mix[i]));
         }
     }
 };
 
 // s_i ^= (s_{i+10} << SH) | (s_{i+11} >> (32-SH)) for the K words i = K p + j of this lane
-template <int K, int SH>
+template <int K, int SH, int PH>
 __device__ __forceinline__ void xs1024_phase_left(uint32_t (&w)[K], const XsMasks<K> &m)
 {
     constexpr int P = 32 / K;
@@ -66,6 +79,8 @@ __device__ __forceinline__ void xs1024_phase_left(uint32_t (&w)[K], const XsMask
         const uint32_t ml = dlo == 0 ? 0xffffffffu : dlo >= P ? 0u : m.down[dlo - D];
         if (dh == dlo) {
             w[j] ^= __funnelshift_l(lo, hi, SH) & mh; // one LOP3: xor with a masked operand
+        } else if (dh == D && dlo == D + 1) {
+            w[j] ^= __funnelshift_l(lo, hi, SH) & m.mix[PH];
         } else {
             w[j] ^= __funnelshift_l(lo & ml, hi & mh, SH);
         }
@@ -73,7 +88,7 @@ __device__ __forceinline__ void xs1024_phase_left(uint32_t (&w)[K], const XsMask
 }
 
 // s_i ^= (s_{i-10} >> SH) | (s_{i-11} << (32-SH))
-template <int K, int SH>
+template <int K, int SH, int PH>
 __device__ __forceinline__ void xs1024_phase_right(uint32_t (&w)[K], const XsMasks<K> &m)
 {
     constexpr int P = 32 / K;
@@ -98,6 +113,8 @@ __device__ __forceinline__ void xs1024_phase_right(uint32_t (&w)[K], const XsMas
         const uint32_t ml = dul == 0 ? 0xffffffffu : dul >= P ? 0u : m.up[dul - D];
         if (duh == dul) {
             w[j] ^= __funnelshift_r(lo, hi, SH) & mh;
+        } else if (dul == D && duh == D + 1) {
+            w[j] ^= __funnelshift_r(lo, hi, SH) & m.mix[PH];
         } else {
             w[j] ^= __funnelshift_r(lo & ml, hi & mh, SH);
         }
@@ -108,9 +125,9 @@ __device__ __forceinline__ void xs1024_phase_right(uint32_t (&w)[K], const XsMas
 template <int K>
 __device__ __forceinline__ void xs1024_update_k(uint32_t (&w)[K], const XsMasks<K> &m)
 {
-    xs1024_phase_left<K, 9>(w, m);   // 329 = 10*32 +  9
-    xs1024_phase_right<K, 27>(w, m); // 347 = 10*32 + 27
-    xs1024_phase_left<K, 24>(w, m);  // 344 = 10*32 + 24
+    xs1024_phase_left<K, 9, 0>(w, m);   // 329 = 10*32 +  9
+    xs1024_phase_right<K, 27, 1>(w, m); // 347 = 10*32 + 27
+    xs1024_phase_left<K, 24, 2>(w, m);  // 344 = 10*32 + 24
 }
 
 // K consecutive 32-bit words, 4K-byte aligned

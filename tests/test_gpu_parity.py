@@ -170,6 +170,42 @@ def test_xs1024_lane_layouts_are_one_generator(K, store):
         g.close()
 
 
+@pytest.mark.parametrize("xsfill", [0, 1, 2, 3], ids=["by_row_length", "one_shot_ctas", "tickets_1_tile", "tickets_2_tiles"])
+@pytest.mark.parametrize("K", [1, 2, 4, 8, 16])
+def test_xs1024_fill_schedules_are_one_generator(K, xsfill):
+    """the TMA fill path of the paper's generator under every work distribution (one short-lived CTA per item;
+    persistent warps drawing items from the handle's ticket counter, one or two tiles per warp): more items than
+    resident warps (so that warps loop and prefetch the next item's state), a ragged last item, several calls on
+    one handle (the ticket base carries over), rows of 32 k and of 4 k' draws, u32 and f32"""
+    resident_warps = 148 * {1: 32, 2: 28, 4: 14, 8: 7, 16: 3}[K]  # the most any variant keeps on a B200
+    S = 32 * K * (2 * resident_warps + 3) + 32 * (K // 2 + 1)      # a warp hosts K instances; last item ragged
+    g, o = pkg.Rng(pkg.RNG_XS1024W, S, 21), oracle.Rng(pkg.RNG_XS1024W, S, 21)
+    g.set_variant("xs1024", K)
+    g.set_variant("xsfill", xsfill)
+    out = dev_u32(S * 64)
+    for n in (64, 36, 64, 4):
+        g.fill_u32(out, n)
+        assert np.array_equal(host(out, S * n), o.fill_u32(n)), (K, xsfill, n)
+    outf = out.view(torch.float32)
+    g.fill_f32(outf, 32)
+    assert np.array_equal(host(out, S * 32), o.fill_f32(32).view(np.uint32))
+    assert g.draws_done == o.draws_done
+    assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
+
+
+def test_xs1024_fill_long_rows_take_the_ping_pong_tiles():
+    """n >= 2048 selects two tiles per warp; a few instances, long ragged rows"""
+    S, n = 32 * 9, 2048 + 36
+    g, o = pkg.Rng(pkg.RNG_XS1024W, S, 5), oracle.Rng(pkg.RNG_XS1024W, S, 5)
+    out = dev_u32(S * n)
+    for _ in range(2):
+        g.fill_u32(out, n)
+        assert np.array_equal(host(out, S * n), o.fill_u32(n))
+    assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
+
+
 # ---------------------------------------------------------------------------------
 # seeding / sharding: a shard [first, first+n_local) of n_total reproduces those rows
 # ---------------------------------------------------------------------------------
