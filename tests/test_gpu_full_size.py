@@ -154,6 +154,51 @@ def test_c5b_ising_L8192_full_lattice(cfg):
     g.close()
 
 
+# ---- SURVEY.md 8(c)-E7 depth: long single calls (PAPER.md:56 application test; BASELINE config 5 "1000 sweeps") -------
+def _long_ising_call(kind, L, n_streams, n_sweeps, seed, lattice_seed, beta):
+    g, o = pkg.Rng(kind, n_streams, seed), oracle.Rng(kind, n_streams, seed)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, lattice_seed)
+    ref = oracle.ising_init_random(L, lattice_seed)
+    tr = torch.empty(n_sweeps, dtype=torch.int64, device="cuda")
+    g.ising_sweep(sp, L, beta, n_sweeps, tr)                       # ONE call, as bench.py issues it
+    tr_o = o.ising_sweep(ref, L, beta, n_sweeps, trace=True)
+    got = tr.cpu().numpy()
+    for t in sorted({1, 2, 10, 100, n_sweeps}):
+        if t <= n_sweeps:
+            assert int(got[t - 1]) == int(tr_o[t - 1]), f"energy after sweep {t}"
+    assert np.array_equal(got, tr_o), "energy trace"
+    assert np.array_equal(sp.cpu().numpy(), ref), "final lattice"
+    assert g.draws_done == o.draws_done == 2 * (L * L // 2 // n_streams) * n_sweeps
+    if g.state_bytes():
+        assert np.array_equal(g.get_state(), o.get_state()), "final generator state"
+    g.close()
+
+
+@pytest.mark.parametrize("cfg", [W.C5B_PHILOX, W.C5B_XORWOW], ids=lambda c: c.name)
+def test_c5b_ising_L8192_100_sweeps_in_one_call(cfg):
+    """the whole 8192^2 lattice through ONE ising_sweep(n_sweeps = 100) call: the 100-entry energy trace, the final
+    lattice and the final generator state equal the oracle's (the oracle needs about a second per sweep)"""
+    _long_ising_call(cfg.kind, cfg.L, cfg.n_streams, 100, cfg.seed, cfg.lattice_seed, cfg.beta)
+
+
+@pytest.mark.parametrize("cfg", [W.C5B_PHILOX, W.C5B_XORWOW], ids=lambda c: c.name)
+def test_c5b_ising_1000_sweeps_in_one_call_L2048(cfg):
+    """the 1000-sweep single call that bench.py times (draw counter and Philox block index growing over 2000
+    half-sweeps, a 1000-entry trace, pack / unpack once around 1000 sweeps), on 1/16 of the lattice area with the
+    same number of sites per stream, so that the oracle finishes in about a minute"""
+    L = 2048
+    _long_ising_call(cfg.kind, L, cfg.n_streams // 16, 1000, cfg.seed, cfg.lattice_seed, cfg.beta)
+
+
+def test_c5b_ising_L8192_1000_sweeps_exactly_as_benched():
+    """BASELINE config 5 to the letter: L = 8192, 1000 sweeps, ONE call (the call bench.py's C5b_xorwow times);
+    the 1000-entry energy trace, the final 64 MiB lattice and the final XORWOW states against the oracle
+    (about four minutes of oracle time; the Philox variant of this call is covered at 100 sweeps above)"""
+    cfg = W.C5B_XORWOW
+    _long_ising_call(cfg.kind, cfg.L, cfg.n_streams, cfg.n_sweeps, cfg.seed, cfg.lattice_seed, cfg.beta)
+
+
 # ---- the widened rows (SURVEY.md 8(f)) at the sizes bench.py times ------------------------------
 @pytest.mark.parametrize("cfg", [W.N1_PHILOX7, W.N1_LCG32, W.N1_LCG64BOTH, W.N4_LFIB521, W.N4_LFIB1279],
                          ids=lambda c: c.name)
