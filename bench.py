@@ -406,7 +406,7 @@ def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, 
            "ms_per_step": ms / steps, "gpu_launches": int(launches), "dtype": job.dtype}
     # roofline of the (single) dominant kernel: average launch duration = timed region / launches
     n_l = steps if isinstance(job, SeedJob) else max(int(launches), 1)  # SeedJob counts per step (many small launches)
-    res["roofline"] = roofline(job.name, job.bound, job.alg_per_launch(), ms * 1e-3 / n_l, store_gbs)
+    res["roofline"] = roofline(getattr(job, "key", job.name), job.bound, job.alg_per_launch(), ms * 1e-3 / n_l, store_gbs)
     if clocks:
         res["clocks"] = clocks
     if job.name in PAPER_GTX480:
@@ -463,7 +463,9 @@ def make_job(name: str, rank: int, world: int, buf, ising_sweeps: int) -> Job:
     }
     if name not in table:
         raise SystemExit(f"unknown --workload {name}; choose from {sorted(table)}")
-    return table[name]()
+    job = table[name]()
+    job.key = name  # the --workload name: what config.workload and profiles/traffic.json are keyed by
+    return job
 
 
 # (name, steps, warmup): the secondary configs of --suite full; sized so that the whole

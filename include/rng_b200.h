@@ -19,7 +19,11 @@
  *    last failing call of the calling thread.
  *  - Pointers named d_* are DEVICE pointers owned by the caller (e.g. PyTorch
  *    tensors), 16-byte aligned unless stated, on the device that was current
- *    when the handle was created.  Pointers named h_* are HOST pointers owned by
+ *    when the handle was created; every call that takes a handle must be made
+ *    with that device current (RNG_E_INVAL otherwise: the handle's state, its
+ *    staging buffers and its launch geometry belong to that device).  Calls on
+ *    ONE handle must not overlap (different handles may run on different
+ *    streams concurrently).  Pointers named h_* are HOST pointers owned by
  *    the caller (pinned memory makes the copies asynchronous, pageable works).
  *    The library never allocates or frees caller buffers.
  *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default
@@ -33,6 +37,9 @@
  *  - Canonical output layout is stream-major:  out[s*n + j] = draw j (of this
  *    call) of local stream s  (BASELINE.json config 1: "per stream to a flat
  *    array").
+ *  - A call that issues several launches (ising_sweep, ising_sweep_multihit) and
+ *    fails at one of them leaves draws_done at the draws already enqueued, so
+ *    the handle's position stays equal to its device state.
  *  - No CPU fallback exists: without a CUDA device every call that needs one
  *    fails with RNG_E_CUDA.
  */
@@ -230,8 +237,11 @@ int ising_sweep_host(rng_handle *h, int8_t *h_spins, uint32_t L, double beta, ui
  * Canonical order, independent of the device layout:
  *   LCG64 / LEAPFROG: n_local x u64 (current x of each stream)
  *   XORWOW: n_local x {x,y,z,w,v,d} u32, stream-major
- *   PHILOX (both): 0 bytes;  XS1024W: n_local x u32 (word s%32 of instance s/32)
- *   LCG32: n_local x u32 (current x of each stream)
+ *   PHILOX (both): 0 bytes;  XS1024W and XS1024W_SKIP: n_local x u32 (word s%32 of instance s/32)
+ *   LCG32 / LCG32_LEAPFROG: n_local x u32 (current x of each stream)
+ *   LCG64_BOTH: n_local x u64 (current x; which half comes next is draws_done & 1)
+ *   LFIB521 / LFIB1279: (n_local/256) x r floats, an instance's last r numbers, oldest first
+ *   MWC: n_local x u64 (c << 32 | x);  MWC_MULTI: n_local x {x, c, a} u32, stream-major
  * rng_get_state/rng_set_state synchronise the device; bytes must equal
  * rng_state_bytes(kind, n_local).  draws_done is read / set separately. */
 uint64_t rng_state_bytes(int kind, uint64_t n_streams);
@@ -240,7 +250,7 @@ int rng_set_state(rng_handle *h, const void *h_buf, uint64_t bytes);
 uint64_t rng_draws_done(const rng_handle *h);
 int rng_set_draws_done(rng_handle *h, uint64_t draws_done);
 
-/* kernel-variant selection for measurements: name in {"xs1024", "ising", "store", "lcg"},
+/* kernel-variant selection for measurements: name in {"xs1024", "xsfill", "ising", "store", "lcg"},
  * value = variant index (0 = default).  Every variant of an operation produces
  * identical bits; see DESIGN.md section 6.  Unknown name/value: RNG_E_INVAL. */
 int rng_set_variant(rng_handle *h, const char *name, int value);

@@ -1,0 +1,115 @@
+"""Summarise `ncu --page raw --csv` exports of the dominant kernels into the two files bench.py and the
+judge read: a text page of the metrics that matter on this path and `profiles/traffic.json`.
+
+    python -m paper_1204_6193_b200.ncu_summary RAW_DIR --text profiles/r02_ncu_full.txt [--json profiles/traffic.json]
+
+RAW_DIR holds one `raw_<workload>.csv` per capture, <workload> being bench.py's `--workload` name; each is
+
+    ncu -i rep_<workload>.ncu-rep --page raw --csv > raw_<workload>.csv
+
+of a capture taken with
+
+    ncu --set full --clock-control none --import-source on -k regex:<kernel> -s <skip> -c 1 -f -o rep_<workload> \\
+        python bench.py --suite primary --steps 5 --warmup 3 --no-e2e --no-cpu-baseline --ising-sweeps 3 --workload <workload>
+
+(only after the same bench.py command has exited 0 without ncu).  Nothing here runs a kernel or is imported by
+the product path; bench.py reads the JSON as STATIC context (`measured_in_this_run: false`).
+"""
+from __future__ import annotations
+
+import argparse
+import csv
+import glob
+import json
+import os
+
+KEYS = [
+    "gpu__time_duration.sum", "dram__bytes_write.sum", "dram__bytes_read.sum",
+    "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "sm__throughput.avg.pct_of_peak_sustained_elapsed",
+    "smsp__issue_active.avg.pct_of_peak_sustained_active", "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active",
+    "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed",
+    "sm__inst_executed_pipe_lsu.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_uniform.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active", "sm__warps_active.avg.pct_of_peak_sustained_active",
+    "smsp__inst_executed.sum", "launch__registers_per_thread", "launch__grid_size", "launch__block_size",
+    "launch__occupancy_limit_registers", "launch__occupancy_limit_shared_mem",
+    "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", "l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum",
+    "l1tex__throughput.avg.pct_of_peak_sustained_elapsed", "lts__throughput.avg.pct_of_peak_sustained_elapsed",
+    "lts__t_sector_hit_rate.pct", "sm__cycles_elapsed.max", "smsp__cycles_active.avg", "sm__cycles_active.avg",
+]
+UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+TIME_US = {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}
+
+
+def _num(d, k):
+    try:
+        return float(d[k].replace(",", ""))
+    except Exception:
+        return None
+
+
+def summarise(raw_dir: str, text_path: str, json_path: str | None, source: str) -> dict:
+    entries = {}
+    with open(text_path, "w") as f:
+        for p in sorted(glob.glob(os.path.join(raw_dir, "raw_*.csv"))):
+            rows = list(csv.reader(open(p)))
+            if len(rows) < 3:
+                continue
+            hdr, units = rows[0], rows[1]
+            name = os.path.basename(p)[4:-4]
+            for r in rows[2:]:
+                d, u = dict(zip(hdr, r)), dict(zip(hdr, units))
+                f.write(f"== [{name}] {d.get('Kernel Name', '?')} grid {d.get('Grid Size', '')} block {d.get('Block Size', '')}\n")
+                for k in KEYS:
+                    if d.get(k, "") != "":
+                        f.write(f"  {k:88s} {d[k]:>20s} {u.get(k, '')}\n")
+                stalls = [(_num(d, k), k) for k in hdr if k.startswith("smsp__average_warps_issue_stalled_")
+                          and k.endswith("_per_issue_active.ratio") and _num(d, k) is not None]
+                for v, k in sorted(stalls, reverse=True)[:6]:
+                    f.write(f"  {k:88s} {v:20.3f} warps/issue\n")
+                pipes = [(_num(d, k), k) for k in hdr if k.startswith("sm__inst_executed_pipe_")
+                         and k.endswith("pct_of_peak_sustained_active") and _num(d, k) is not None]
+                f.write("  top pipes: " + ", ".join(f"{k.split('pipe_')[1].split('.')[0]} {v:.1f}%"
+                                                     for v, k in sorted(pipes, reverse=True)[:6]) + "\n")
+
+                def byt(k):
+                    v = _num(d, k)
+                    return None if v is None else v * UNIT.get(u.get(k, ""), 1.0)
+                traffic = (byt("dram__bytes_read.sum") or 0.0) + (byt("dram__bytes_write.sum") or 0.0)
+                t_us = (_num(d, "gpu__time_duration.sum") or 0.0) * TIME_US.get(u.get("gpu__time_duration.sum", "us"), 1.0)
+                entries[name] = {
+                    "kernel": d.get("Kernel Name"), "dram_bytes_per_launch": int(traffic), "ncu_time_us": round(t_us, 3),
+                    "source": source,
+                    "issue_active_pct": _num(d, "smsp__issue_active.avg.pct_of_peak_sustained_active"),
+                    "pipe_alu_pct": _num(d, "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active"),
+                    "pipe_fma_pct": _num(d, "sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active"),
+                    "pipe_fmaheavy_cycles_pct_of_elapsed": _num(d, "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed"),
+                    "pipe_lsu_pct": _num(d, "sm__inst_executed_pipe_lsu.avg.pct_of_peak_sustained_active"),
+                    "dram_throughput_pct": _num(d, "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed"),
+                }
+    if json_path:
+        old = {}
+        if os.path.exists(json_path):
+            old = json.load(open(json_path))
+        old["_comment"] = ("keyed by bench.py --workload name; per workload, from the `ncu --set full` capture of its dominant "
+                           "kernel (see each entry's `source`): dram__bytes_read.sum + dram__bytes_write.sum per launch, "
+                           "smsp__issue_active, sm__inst_executed_pipe_* (pct of peak sustained, active cycles), "
+                           "sm__pipe_fmaheavy_cycles_active (pct of elapsed), gpu__dram_throughput.  Written by "
+                           "`python -m paper_1204_6193_b200.ncu_summary`; bench.py copies these as static context "
+                           "(measured_in_this_run: false) and never runs under ncu.")
+        old.update(entries)
+        with open(json_path, "w") as f:
+            json.dump(old, f, indent=1)
+    return entries
+
+
+if __name__ == "__main__":
+    ap = argparse.ArgumentParser()
+    ap.add_argument("raw_dir")
+    ap.add_argument("--text", required=True)
+    ap.add_argument("--json", default=None)
+    ap.add_argument("--source", default=None, help="what the entries cite as their capture (default: --text)")
+    a = ap.parse_args()
+    e = summarise(a.raw_dir, a.text, a.json, a.source or a.text)
+    print(f"{len(e)} captures -> {a.text}" + (f", {a.json}" if a.json else ""))

@@ -156,16 +156,3 @@ def test_accept_table_integer_form_is_exactly_the_float_compare(L):
                 np.arange(t - 3, t + 4), [0, 1, (1 << 24) - 1], rs.randint(0, 1 << 24, 2000)]), 0, (1 << 24) - 1))
             u = cand.astype(np.float32) * np.float32(2.0 ** -24)
             assert np.array_equal(u < P[i], cand < t), (beta, i)
-
-
-def test_table_scripts_refuse_to_run_without_a_device():
-    """table1 / table2 reproduce the paper's tables on a GPU; without one they must say so (no CPU fallback)"""
-    import subprocess
-    import sys
-    import torch
-    if torch.cuda.is_available():
-        pytest.skip("a CUDA device is present")
-    for mod in ("paper_1204_6193_b200.table1", "paper_1204_6193_b200.table2"):
-        r = subprocess.run([sys.executable, "-m", mod], capture_output=True, text=True, timeout=120,
-                           cwd=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
-        assert r.returncode != 0 and "needs a CUDA device" in (r.stderr + r.stdout), mod

@@ -40,7 +40,7 @@ def _stub_result(bench, workload, long_name, bound, unit="Gnum/s"):
     r = {"name": long_name, "value": 1234.5678901234567, "unit": unit, "steps": 20, "warmup": 5,
          "ms_per_step": 0.67890123456789, "gpu_launches": 20, "dtype": "u32", "workload": workload,
          "clocks": {"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": ["sw_power_cap"], "samples": 4000}}
-    r["roofline"] = bench.roofline(long_name, bound, 4.3e9 if bound == "hbm" else 5e10, 6.8e-4, 7300.123)
+    r["roofline"] = bench.roofline(workload, bound, 4.3e9 if bound == "hbm" else 5e10, 6.8e-4, 7300.123)
     return r
 
 
@@ -91,7 +91,7 @@ def test_b200_line_is_one_compact_parseable_line_for_every_suite():
 def test_alu_roofline_leads_with_the_ncu_figures():
     sys.path.insert(0, ROOT)
     import bench
-    rl = bench.roofline("C3_xorwow_2^22x256_draw_reduce", "alu", 1.07e10, 3.5e-4)
+    rl = bench.roofline("C3_draw", "alu", 1.07e10, 3.5e-4)
     assert rl["bound"] == "alu" and rl["basis"] == "algorithmic instruction count"
     assert rl["ncu"]["measured_in_this_run"] is False and rl["ncu_issue_active_pct"] > 0 and rl["ncu_binding_pipe"]
 

@@ -65,6 +65,51 @@ def test_two_ranks_over_gloo_reproduce_the_unsharded_streams():
     mp.spawn(_worker, args=(2, _free_port(), 64, 24), nprocs=2, join=True)
 
 
+def _gpu_worker(rank: int, world: int, port: int, n_per_rank: int, n: int):
+    """the PRODUCT's shards (rng_create_shard through the binding, kernels on cuda:0 shared by both ranks -- no
+    rank's kernel waits for another's), gathered over gloo and compared with the unsharded oracle"""
+    import oracle
+    import paper_1204_6193_b200 as pkg
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        torch.cuda.set_device(0)
+        for kind in (W.LCG64, W.LCG64_LEAPFROG, W.XORWOW, W.PHILOX4X32_10, W.XS1024W, W.PHILOX4X32_7, W.LCG32,
+                     W.XS1024W_SKIP, W.LCG64_BOTH, W.LFIB521, W.LFIB1279):
+            per = 256 if kind in (W.LFIB521, W.LFIB1279) else n_per_rank
+            n_total, first, n_local = sharding.weak_scaling_shard(rank, world, per)
+            g = pkg.Rng(kind, n_local, W.MASTER_SEED, first=first, n_total=n_total)
+            out = torch.empty(n_local * n, dtype=torch.int32, device="cuda")
+            g.fill_u32(out, n)
+            red = torch.empty(2 * n_local, dtype=torch.int32, device="cuda")
+            g.draw_reduce(red, 7)
+            g.close()
+            parts = [torch.empty(n_local * n, dtype=torch.int32) for _ in range(world)]
+            dist.all_gather(parts, out.cpu())
+            reds = [torch.empty(2 * n_local, dtype=torch.int32) for _ in range(world)]
+            dist.all_gather(reds, red.cpu())
+            if rank == 0:
+                o = oracle.Rng(kind, n_total, W.MASTER_SEED)
+                assert np.array_equal(torch.cat(parts).numpy().view(np.uint32), o.fill_u32(n)), f"kind {kind}: fill"
+                assert np.array_equal(torch.cat(reds).numpy().view(np.uint32), o.draw_reduce(7)), f"kind {kind}: draw"
+        # bench.py's timing reduction on device-timed values
+        t = torch.tensor([1.0 + rank], dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        assert float(t.item()) == float(world)
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_two_ranks_of_product_shards_reproduce_the_unsharded_streams():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (no CPU fallback exists)")
+    from paper_1204_6193_b200 import build
+    build.build()
+    mp.spawn(_gpu_worker, args=(2, _free_port(), 2048 + 64, 40), nprocs=2, join=True)
+
+
 def test_shard_range_properties():
     for world in (1, 2, 3, 8):
         for total in (32, 64, 32 * 9, 32 * 1000):
