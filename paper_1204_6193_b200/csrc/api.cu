@@ -201,6 +201,7 @@ int rng_destroy(rng_handle *h)
     if (h->staging) cudaFree(h->staging);
     if (h->energy_scratch) cudaFree(h->energy_scratch);
     if (h->ms_planes) cudaFree(h->ms_planes);
+    if (h->mh_mailbox) cudaFree(h->mh_mailbox);
     delete h;
     return RNG_OK;
 }
@@ -331,6 +332,24 @@ int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta
     ising_accept_table(beta, nullptr, tab.T);
     cudaStream_t st = (cudaStream_t)stream;
     uint64_t d = h->g.draws_done;
+    if (n_sweeps == 0) return RNG_OK;
+    // variant "ising": 0 = automatic (the whole call in ONE cooperative launch where that is faster: no energy trace
+    // asked for, every tile resident, few hits -- PAPER.md:58's k = 1 regime without its launches and its per-visit
+    // state traffic), 1 = always one launch per coarse colour, 4 = one launch whenever the call qualifies.
+    // Same trajectory either way.
+    if (!d_trace && h->var_ising != 1 && ising_multihit_coop_eligible(*h, L, tile, k_hits, n_sweeps, h->var_ising == 4)) {
+        const uint64_t need = (uint64_t)(L / tile) * (L / tile) * 4ull * sizeof(unsigned long long);
+        if (h->mh_mailbox_bytes < need) {
+            if (h->mh_mailbox) cudaFree(h->mh_mailbox);
+            h->mh_mailbox = nullptr;
+            h->mh_mailbox_bytes = 0;
+            CU(cudaMalloc((void **)&h->mh_mailbox, need));
+            h->mh_mailbox_bytes = need;
+        }
+        CU(launch_ising_multihit_coop(*h, d_spins, L, tab, tile, k_hits, n_sweeps, d, h->mh_mailbox, st));
+        h->g.draws_done = d + per_sweep * n_sweeps;
+        return RNG_OK;
+    }
     for (uint32_t t = 0; t < n_sweeps; t++) {
         for (int c = 0; c < 2; c++) {
             CU_AT(launch_ising_multihit(*h, d_spins, L, tab, tile, k_hits, d, c, st), h, d);

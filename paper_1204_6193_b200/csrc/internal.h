@@ -56,6 +56,8 @@ struct rng_handle {
     mutable uint64_t ticket_base;
     uint32_t *ms_planes;     // device scratch of the multi-spin Ising path: two bit planes of L*L/64 words
     uint64_t ms_planes_bytes;
+    unsigned long long *mh_mailbox; // device scratch of the one-launch multi-hit path: (L/T)^2 * 4 halo words
+    uint64_t mh_mailbox_bytes;
     int var_xs1024, var_ising, var_store, var_lcg, var_xsfill;
     int api_kind; // the kind rng_create was called with (g.kind is RNG_XS1024W for RNG_XS1024W_SKIP)
 };
@@ -149,6 +151,11 @@ cudaError_t launch_ising_ms_half_sweep(const rng_handle &h, uint32_t *planes, ui
 // ising_mh.cu (the paper's double-checkerboard multi-hit kernel; one launch per coarse colour)
 cudaError_t launch_ising_multihit(const rng_handle &h, int8_t *d_spins, uint32_t L, const IsingTable &tab, uint32_t T,
                                   uint32_t k_hits, uint64_t draws_done, int coarse, cudaStream_t st);
+// the whole ising_sweep_multihit call in one cooperative launch (tiles resident in shared memory, mailbox halos)
+bool ising_multihit_coop_eligible(const rng_handle &h, uint32_t L, uint32_t T, uint32_t k_hits, uint32_t n_sweeps, bool force);
+cudaError_t launch_ising_multihit_coop(const rng_handle &h, int8_t *d_spins, uint32_t L, const IsingTable &tab, uint32_t T,
+                                       uint32_t k_hits, uint32_t n_sweeps, uint64_t draws_done, unsigned long long *mailbox,
+                                       cudaStream_t st);
 cudaError_t launch_ising_init_random(int8_t *d_spins, uint32_t L, uint64_t seed, cudaStream_t st);
 cudaError_t launch_ising_energy(const int8_t *d_spins, uint32_t L, int64_t *d_out, cudaStream_t st);
 

@@ -591,6 +591,48 @@ def test_ising_multihit_bit_exact(kind, L, T, k, sweeps):
     g.close()
 
 
+@pytest.mark.parametrize("kind", KINDS, ids=IDS)
+@pytest.mark.parametrize("L,T,k,sweeps", [(16, 8, 1, 5), (32, 8, 7, 3), (64, 16, 2, 4), (128, 32, 5, 2), (96, 16, 100, 1),
+                                          (256, 16, 1, 9), (512, 16, 3, 2), (1024, 16, 1, 3), (1024, 8, 1, 2)])
+def test_ising_multihit_whole_call_in_one_launch_bit_exact(kind, L, T, k, sweeps):
+    """the whole call as ONE cooperative launch (tiles stay in shared memory, generator states in registers, halos
+    travel as 64-bit words between the inboxes of neighbouring tiles; variant "ising" = 4 takes this path whenever
+    the call qualifies, the default only where it measured faster).  Same trajectory as one launch per coarse colour
+    (variant 1); two calls per handle (stage numbers restart, the streams continue); L = 1024 makes every thread
+    serve two streams"""
+    S = L * L // 4
+    if kind in LFIB_KINDS:
+        pytest.skip("ring shared by a 256-thread CTA: per-colour launches only (covered by test_ising_multihit_bit_exact)")
+    beta = 0.4
+    g, o = pkg.Rng(kind, S, 17), oracle.Rng(kind, S, 17)
+    g2 = pkg.Rng(kind, S, 17)
+    g.set_variant("ising", 4)
+    g2.set_variant("ising", 1)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, 9)
+    sp2 = sp.clone()
+    sp_o = oracle.ising_init_random(L, 9)
+    e = torch.zeros(1, dtype=torch.int64, device="cuda")
+    for call in range(2):
+        l1 = pkg.rng_kernel_launches()
+        g.ising_sweep_multihit(sp, L, beta, sweeps, T, k)
+        assert pkg.rng_kernel_launches() - l1 == 1, "expected the one-launch path"
+        g2.ising_sweep_multihit(sp2, L, beta, sweeps, T, k)
+        o.ising_sweep_multihit(sp_o, L, beta, sweeps, T, k)
+        assert np.array_equal(sp.cpu().numpy(), sp_o), f"call {call}: lattice"
+        assert np.array_equal(sp2.cpu().numpy(), sp_o), f"call {call}: lattice (per-colour launches)"
+        pkg.ising_energy(sp, L, e)
+        assert int(e.item()) == oracle.ising_energy(sp_o, L)
+    assert g.draws_done == o.draws_done == 2 * 4 * k * sweeps
+    if g.state_bytes():
+        assert np.array_equal(g.get_state(), o.get_state())
+    out = dev_u32(S * 3)
+    g.fill_u32(out, 3)
+    assert np.array_equal(host(out, S * 3), o.fill_u32(3))
+    g.close()
+    g2.close()
+
+
 def test_ising_multihit_argument_errors():
     g = pkg.Rng(pkg.RNG_PHILOX4X32_10, 16, 1)
     sp = torch.ones(64, dtype=torch.int8, device="cuda")
