@@ -250,7 +250,7 @@ int rng_set_state(rng_handle *h, const void *h_buf, uint64_t bytes);
 uint64_t rng_draws_done(const rng_handle *h);
 int rng_set_draws_done(rng_handle *h, uint64_t draws_done);
 
-/* kernel-variant selection for measurements: name in {"xs1024", "xsfill", "ising", "store", "lcg"},
+/* kernel-variant selection for measurements: name in {"xs1024", "xsfill", "ising", "store", "lcg", "cvt"},
  * value = variant index (0 = default).  Every variant of an operation produces
  * identical bits; see DESIGN.md section 6.  Unknown name/value: RNG_E_INVAL. */
 int rng_set_variant(rng_handle *h, const char *name, int value);

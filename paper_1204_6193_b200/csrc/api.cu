@@ -494,6 +494,7 @@ int rng_set_variant(rng_handle *h, const char *name, int value)
     else if (!strcmp(name, "store")) h->var_store = value;
     else if (!strcmp(name, "lcg")) h->var_lcg = value;
     else if (!strcmp(name, "xsfill")) h->var_xsfill = value;
+    else if (!strcmp(name, "cvt")) h->var_cvt = value;
     else return fail(RNG_E_INVAL, "rng_set_variant: unknown name '%s'", name);
     return RNG_OK;
 }

@@ -76,9 +76,19 @@ __global__ void __launch_bounds__(256) philox_fill_kernel(uint32_t *__restrict__
 //    its IMAD.WIDE arithmetic, not by an uneven share of the write bandwidth, and same-address atomics cost
 //    about 3 ns each.
 // ------------------------------------------------------------------------------------
+// the four words of a block as they are stored: the draws, or the bits of their float images (form CVT of the
+// fixed map, generators.cuh)
+template <bool F32, int CVT>
+__device__ __forceinline__ uint4 philox_out(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3)
+{
+    if (!F32) return make_uint4(c0, c1, c2, c3);
+    return make_uint4(__float_as_uint(u32_to_f32_form<CVT>(c0)), __float_as_uint(u32_to_f32_form<CVT>(c1)),
+                      __float_as_uint(u32_to_f32_form<CVT>(c2)), __float_as_uint(u32_to_f32_form<CVT>(c3)));
+}
+
 // U independent 4-word blocks per lane (blocks rb0, rb0+32, ...), ten rounds interleaved,
 // one 128-bit streaming store each.  CHECK = bounds-check each block (ragged last tile).
-template <bool F32, int U, bool CHECK, int R>
+template <bool F32, int U, bool CHECK, int R, int CVT>
 __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_t b0, uint32_t rb0,
                                              uint32_t blocks_per_row, const uint32_t (&rk0)[R],
                                              const uint32_t (&rk1)[R])
@@ -110,9 +120,7 @@ __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_
 #pragma unroll
     for (int u = 0; u < U; u++) {
         if (!CHECK || rb0 + 32u * u < blocks_per_row) {
-            const uint4 v = make_uint4(out_word_cvt(c0[u], F32), out_word_cvt(c1[u], F32), out_word_cvt(c2[u], F32),
-                                       out_word_cvt(c3[u], F32));
-            __stcs(dst + 32 * u, v); // streaming 128-bit store
+            __stcs(dst + 32 * u, philox_out<F32, CVT>(c0[u], c1[u], c2[u], c3[u])); // streaming 128-bit store
         }
     }
 }
@@ -128,14 +136,21 @@ __device__ __forceinline__ void philox_group(uint32_t *__restrict__ row, uint64_
 //    the same for every block of the tile: one product per lane and group (`q`).
 // Rounds 3..R are the generic round.  Same bits as philox4x32<R> (tests compare both paths
 // with the oracle, also across a 2^32-block boundary).
-template <bool F32, int U, int R>
+template <bool F32, int U, int R, int CVT>
 __device__ __forceinline__ void philox_group_fast(uint32_t *__restrict__ row, uint32_t blo, uint32_t bhi, uint32_t rb0,
                                                   const uint32_t (&rk0)[R], const uint32_t (&rk1)[R])
 {
-    static_assert(R >= 2, "needs two rounds");
+    static_assert(R >= 3, "needs three rounds");
     uint32_t c0[U], c1[U], c2[U], c3[U];
     const uint64_t p00 = (uint64_t)kPhM0 * blo;                       // round 1, block u = 0
     const uint64_t q = (uint64_t)kPhM0 * (bhi ^ rk0[0]);              // round 2, first S-box: tile-uniform input
+    // q and the round keys are warp-uniform: fold them into ONE uniform operand per xor here, because a LOP3
+    // takes a single uniform-register source and ptxas otherwise copies the second one into a vector register
+    // for every block (12 IMAD.U32 per group of 8 blocks in round 1's build)
+    uint32_t hq1 = (uint32_t)(q >> 32) ^ rk1[1];                      // round 2: c2 = hi(q) ^ a3 ^ k1'
+    uint32_t lq2 = (uint32_t)q ^ rk1[2];                              // round 3: c2 = hi(p0) ^ c3 ^ k1'', c3 = lo(q)
+    hq1 = __shfl_sync(0xffffffffu, hq1, 0);                           // (a shuffle is opaque to the xor re-association
+    lq2 = __shfl_sync(0xffffffffu, lq2, 0);                           //  of nvvm and ptxas, which would unfold them)
     constexpr uint64_t STEP = 32ull * kPhM0;
 #pragma unroll
     for (int u = 0; u < U; u++) {
@@ -145,13 +160,18 @@ __device__ __forceinline__ void philox_group_fast(uint32_t *__restrict__ row, ui
         const uint32_t a3 = (uint32_t)p0;
         // round 2
         const uint64_t p1 = (uint64_t)kPhM1 * a2;
-        c0[u] = (uint32_t)(p1 >> 32) ^ rk0[1];                        // ^ c1 (= 0)
-        c2[u] = (uint32_t)(q >> 32) ^ a3 ^ rk1[1];
-        c1[u] = (uint32_t)p1;
-        c3[u] = (uint32_t)q;
+        const uint32_t b0 = (uint32_t)(p1 >> 32) ^ rk0[1];            // ^ c1 (= 0)
+        const uint32_t b2 = hq1 ^ a3;
+        // round 3 (c3 = lo(q) is uniform and already folded into lq2)
+        const uint64_t r0 = (uint64_t)kPhM0 * b0;
+        const uint64_t r1 = (uint64_t)kPhM1 * b2;
+        c0[u] = (uint32_t)(r1 >> 32) ^ (uint32_t)p1 ^ rk0[2];
+        c2[u] = (uint32_t)(r0 >> 32) ^ lq2;
+        c1[u] = (uint32_t)r1;
+        c3[u] = (uint32_t)r0;
     }
 #pragma unroll
-    for (int r = 2; r < R; r++) {
+    for (int r = 3; r < R; r++) {
 #pragma unroll
         for (int u = 0; u < U; u++) {
             const uint64_t p0 = (uint64_t)kPhM0 * c0[u];
@@ -167,13 +187,13 @@ __device__ __forceinline__ void philox_group_fast(uint32_t *__restrict__ row, ui
     uint4 *dst = reinterpret_cast<uint4 *>(row) + rb0;
 #pragma unroll
     for (int u = 0; u < U; u++) {
-        const uint4 v = make_uint4(out_word_cvt(c0[u], F32), out_word_cvt(c1[u], F32), out_word_cvt(c2[u], F32),
-                                   out_word_cvt(c3[u], F32));
-        __stcs(dst + 32 * u, v);
+        __stcs(dst + 32 * u, philox_out<F32, CVT>(c0[u], c1[u], c2[u], c3[u]));
     }
 }
 
-template <bool F32, int U, int T, int R>
+// ALLFAST (host-checked: every tile is full and no tile of the call crosses a 2^32-block boundary): the per-tile
+// bookkeeping shrinks to the key schedule and the row pointer.
+template <bool F32, int U, int T, int R, bool ALLFAST, int CVT>
 __global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restrict__ out, uint64_t first, uint64_t seed,
                                                               uint64_t b0, uint64_t n, uint32_t blocks_per_row,
                                                               uint32_t tiles_per_row, uint64_t n_tiles)
@@ -196,6 +216,20 @@ __global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restr
             rk1[r] = (uint32_t)(key >> 32) + (uint32_t)r * kPhW1;
         }
         uint32_t *row = out + s * n;
+        if (ALLFAST) {
+#pragma unroll 1
+            for (int g = 0; g < T; g++) {
+                const uint32_t rb0 = (c * T + g) * (32u * U) + lane;
+                philox_group_fast<F32, U, R, CVT>(row, (uint32_t)b0 + rb0, (uint32_t)(b0 >> 32), rb0, rk0, rk1);
+            }
+            s += ds;
+            c += dc;
+            if (c >= tiles_per_row) {
+                c -= tiles_per_row;
+                s++;
+            }
+            continue;
+        }
         const bool tile_full = (uint64_t)(c + 1u) * (T * 32u * U) <= (uint64_t)blocks_per_row; // warp-uniform
         // first and last block index of the tile (warp-uniform); equal high words <=> lo32 does not wrap
         const uint64_t bt0 = b0 + (uint64_t)c * (T * 32u * U), bt1 = bt0 + (T * 32u * U - 1u);
@@ -203,16 +237,16 @@ __global__ void __launch_bounds__(256) philox_fill_warp_kernel(uint32_t *__restr
 #pragma unroll 1
             for (int g = 0; g < T; g++) {
                 const uint32_t rb0 = (c * T + g) * (32u * U) + lane;
-                philox_group_fast<F32, U, R>(row, (uint32_t)b0 + rb0, (uint32_t)(bt0 >> 32), rb0, rk0, rk1);
+                philox_group_fast<F32, U, R, CVT>(row, (uint32_t)b0 + rb0, (uint32_t)(bt0 >> 32), rb0, rk0, rk1);
             }
         } else if (tile_full) {
 #pragma unroll 1
             for (int g = 0; g < T; g++)
-                philox_group<F32, U, false, R>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
+                philox_group<F32, U, false, R, CVT>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
         } else {
 #pragma unroll 1
             for (int g = 0; g < T; g++)
-                philox_group<F32, U, true, R>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
+                philox_group<F32, U, true, R, CVT>(row, b0, (c * T + g) * (32u * U) + lane, blocks_per_row, rk0, rk1);
         }
         s += ds;
         c += dc;
@@ -396,7 +430,7 @@ static cudaError_t launch_rowtile(const Gen &g, void *d_out, uint64_t n, bool f3
     return cudaGetLastError();
 }
 
-template <bool F32, int U, int T, int R>
+template <bool F32, int U, int T, int R, int CVT = 0>
 static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uint64_t blocks_per_row, cudaStream_t st)
 {
     const uint64_t tpr = (blocks_per_row + 32 * U * T - 1) / (32 * U * T);
@@ -405,21 +439,30 @@ static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uin
     static int per_sm = 0; // a property of the kernel on sm_100a; the same on every device this library targets
     if (!per_sm) {
         int b = 0;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, philox_fill_warp_kernel<F32, U, T, R>, 256, 0);
+        cudaError_t e =
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, philox_fill_warp_kernel<F32, U, T, R, false, CVT>, 256, 0);
         if (e != cudaSuccess) return e;
         per_sm = b > 0 ? b : 1;
     }
     uint64_t grid = (uint64_t)sm_count() * per_sm;
     const uint64_t need = (n_tiles + 7) / 8;
     if (grid > need) grid = need;
-    philox_fill_warp_kernel<F32, U, T, R><<<(unsigned)grid, 256, 0, st>>>(o, g.first, g.seed, g.draws_done >> 2, n,
-                                                                     (uint32_t)blocks_per_row, (uint32_t)tpr, n_tiles);
+    const uint64_t b0 = g.draws_done >> 2;
+    // every tile full, and the call's blocks share the high counter word: the lean per-tile path
+    const bool allfast = blocks_per_row % (32 * U * T) == 0 && (b0 >> 32) == ((b0 + blocks_per_row - 1) >> 32);
+    if (allfast)
+        philox_fill_warp_kernel<F32, U, T, R, true, CVT><<<(unsigned)grid, 256, 0, st>>>(o, g.first, g.seed, b0, n,
+                                                                              (uint32_t)blocks_per_row, (uint32_t)tpr, n_tiles);
+    else
+        philox_fill_warp_kernel<F32, U, T, R, false, CVT><<<(unsigned)grid, 256, 0, st>>>(o, g.first, g.seed, b0, n,
+                                                                               (uint32_t)blocks_per_row, (uint32_t)tpr, n_tiles);
     count_launch();
     return cudaGetLastError();
 }
 
 template <int R>
-static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, bool f32, int variant, cudaStream_t st)
+static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, bool f32, int variant, int cvt,
+                                      cudaStream_t st)
 {
     const uint64_t d0 = g.draws_done;
     const uint64_t blocks_per_row = ((d0 + n - 1) >> 2) - (d0 >> 2) + 1;
@@ -428,6 +471,13 @@ static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, boo
     if (aligned && blocks_per_row <= 0x7fffffffull) {
 #define PW(U, T) (f32 ? launch_philox_warp<true, U, T, R>(g, o, n, blocks_per_row, st) \
                       : launch_philox_warp<false, U, T, R>(g, o, n, blocks_per_row, st))
+        if (f32 && variant == 0 && cvt >= 1 && cvt <= 3) { // variant "cvt": the float map in another exact form
+            switch (cvt) {
+            case 1: return launch_philox_warp<true, 8, 1, R, 1>(g, o, n, blocks_per_row, st);
+            case 2: return launch_philox_warp<true, 8, 1, R, 2>(g, o, n, blocks_per_row, st);
+            default: return launch_philox_warp<true, 8, 1, R, 3>(g, o, n, blocks_per_row, st);
+            }
+        }
         switch (variant) { // identical bits; (U, T) = blocks interleaved per lane, groups per tile
         case 1: return PW(4, 2);
         case 2: return PW(2, 4);
@@ -467,8 +517,8 @@ cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, 
     case RNG_XS1024W:
         if (h.var_xs1024 == 64) return launch_rowtile<RNG_XS1024W>(g, d_out, n, f32, h.var_store, st);
         return launch_xs1024_fill(h, d_out, n, f32, st);
-    case RNG_PHILOX4X32_10: return launch_philox_fill<10>(g, d_out, n, f32, h.var_store, st);
-    case RNG_PHILOX4X32_7: return launch_philox_fill<7>(g, d_out, n, f32, h.var_store, st);
+    case RNG_PHILOX4X32_10: return launch_philox_fill<10>(g, d_out, n, f32, h.var_store, h.var_cvt, st);
+    case RNG_PHILOX4X32_7: return launch_philox_fill<7>(g, d_out, n, f32, h.var_store, h.var_cvt, st);
     case RNG_LCG32: return launch_rowtile<RNG_LCG32>(g, d_out, n, f32, h.var_store, st);
     case RNG_LCG64_BOTH: return launch_rowtile<RNG_LCG64_BOTH>(g, d_out, n, f32, h.var_store, st);
     case RNG_LCG32_LEAPFROG: return launch_rowtile<RNG_LCG32_LEAPFROG>(g, d_out, n, f32, h.var_store, st);

@@ -164,28 +164,41 @@ __host__ __device__ __forceinline__ uint32_t xs1024_weyl_term(uint64_t n_updates
     return y ^ (y >> 16);
 }
 
-// fixed output map (BASELINE.json): (u >> 8) * 2^-24, exact (24-bit integer -> float)
-// Evaluated without the integer->float conversion unit (I2FP issues at a quarter of the FFMA
-// rate on sm_100a and shares a pipe with Philox's IMAD.WIDE): with u = b3 b2 b1 b0 (bytes),
-//   A = 0x4B00'b3b2 = 2^23 + (u >> 16),   B = 0x4B00'00b1 = 2^23 + ((u >> 8) & 255)   (one PRMT each)
-//   f = fma(B, 2^-24, fma(A, 2^-16, -128.5))
-// The inner fma is (u>>16) 2^-16 - 1/2 and the outer one adds 1/2 + b1 2^-24; both results
-// are representable, so no rounding occurs anywhere and f == (float)(u >> 8) * 2^-24 bit for bit.
+// fixed output map (BASELINE.json): (u >> 8) * 2^-24, exact (24-bit integer -> float).
+// Evaluated WITHOUT an integer->float conversion: the bit pattern x = u >> 8 < 2^24, read as a float, IS the number
+// x 2^-149 -- below 2^23 a denormal (no implicit one), from 2^23 on the first normal binade, whose exponent bit
+// contributes exactly the 2^23 at which the denormals stop.  One multiplication by 2^125 (exact: x has 24 bits and
+// the product is a normal number) gives x 2^-24.  That is ONE integer-side instruction (the shift) and one FMUL,
+// which the fma-lite pipe takes; the kernels here are bound by integer-side issue, where the
+// conversion instruction I2FP (alu pipe) or two PRMT cost twice as much.  mul.rn.f32 without .ftz: denormal inputs
+// are honoured whatever -ftz the file is compiled with.
 __device__ __forceinline__ float u32_to_f32(uint32_t u)
 {
-    const float A = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7432));
-    const float B = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7441));
-    return __fmaf_rn(B, 0x1p-24f, __fmaf_rn(A, 0x1p-16f, -128.5f));
+    float f;
+    asm("mul.rn.f32 %0, %1, 0f7E000000;" : "=f"(f) : "f"(__uint_as_float(u >> 8))); // 0f7E000000 = 2^125
+    return f;
+}
+// The same map in the other exact forms this library went through, kept selectable in the Philox fill (variant
+// "cvt") so that the difference stays measurable:
+//  1: through the conversion instruction, I2FP(u >> 8) * 2^-24 (I2FP issues on the alu pipe);
+//  2: by exponent bias, A = 0x4B00'b3b2 = 2^23 + (u >> 16), B = 0x4B00'00b1 = 2^23 + ((u >> 8) & 255) (one PRMT each),
+//     f = fma(B, 2^-24, fma(A, 2^-16, -128.5)): the inner fma is (u>>16) 2^-16 - 1/2, the outer one adds
+//     1/2 + b1 2^-24; both results are representable, no rounding occurs;
+//  3: "round up" selects the conversion unit's I2F (xu pipe) for u & ~255 (at most 24 significant bits: exact in
+//     any rounding mode), scaled by 2^-32.
+template <int CVT>
+__device__ __forceinline__ float u32_to_f32_form(uint32_t u)
+{
+    if (CVT == 1) return __uint2float_rn(u >> 8) * 0x1p-24f;
+    if (CVT == 2) {
+        const float A = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7432));
+        const float B = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7441));
+        return __fmaf_rn(B, 0x1p-24f, __fmaf_rn(A, 0x1p-16f, -128.5f));
+    }
+    if (CVT == 3) return __uint2float_ru(u & 0xffffff00u) * 0x1p-32f;
+    return u32_to_f32(u);
 }
 // the 32-bit word a fill kernel stores: the draw itself, or the bits of its float image
-// the same map through the conversion unit: u >> 8 < 2^24 converts exactly, the scaling is a power of two.
-// Measured in the Philox fill (whose fma pipes are the busy ones): 750 us per 4 GiB against 779 us with the
-// PRMT/FFMA form above, so that kernel converts this way; everywhere else the form above is used.
-__device__ __forceinline__ float u32_to_f32_cvt(uint32_t u) { return __uint2float_rn(u >> 8) * 0x1p-24f; }
-__device__ __forceinline__ uint32_t out_word_cvt(uint32_t u, bool f32)
-{
-    return f32 ? __float_as_uint(u32_to_f32_cvt(u)) : u;
-}
 __device__ __forceinline__ uint32_t out_word(uint32_t u, bool f32)
 {
     return f32 ? __float_as_uint(u32_to_f32(u)) : u;

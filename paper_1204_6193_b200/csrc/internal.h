@@ -58,7 +58,7 @@ struct rng_handle {
     uint64_t ms_planes_bytes;
     unsigned long long *mh_mailbox; // device scratch of the one-launch multi-hit path: (L/T)^2 * 4 halo words
     uint64_t mh_mailbox_bytes;
-    int var_xs1024, var_ising, var_store, var_lcg, var_xsfill;
+    int var_xs1024, var_ising, var_store, var_lcg, var_xsfill, var_cvt;
     int api_kind; // the kind rng_create was called with (g.kind is RNG_XS1024W for RNG_XS1024W_SKIP)
 };
 

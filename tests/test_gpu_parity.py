@@ -80,6 +80,41 @@ def test_fill_f32_bit_patterns(kind):
     g.close()
 
 
+def test_f32_map_exact_for_every_24_bit_value():
+    """The library evaluates (u >> 8) 2^-24 by reading u >> 8 as a (denormal) float and multiplying by 2^125
+    (generators.cuh).  Every one of the 2^24 values of u >> 8, each with a different low byte, goes through the
+    fill kernel: an LCG32 stream's first draw is its state word, and rng_set_state chooses the states.  Compared
+    with the oracle's map applied to the same words and with the definition evaluated by numpy."""
+    S = 1 << 24
+    u = (np.arange(S, dtype=np.uint32) << np.uint32(8)) | ((np.arange(S, dtype=np.uint32) * np.uint32(167)) & np.uint32(255))
+    g = pkg.Rng(pkg.RNG_LCG32, S, 1)
+    g.set_state(u)
+    out = torch.empty(S, dtype=torch.float32, device="cuda")
+    g.fill_f32(out, 1)
+    got = out.cpu().numpy()
+    g.close()
+    exp = (u >> np.uint32(8)).astype(np.float32) * np.float32(2.0 ** -24)  # exact: 24-bit integer, power of two
+    assert np.array_equal(got.view(np.uint32), exp.view(np.uint32)), np.flatnonzero(got != exp)[:8]
+    for i in (0, 1, 255, 256, (1 << 23) - 1, 1 << 23, (1 << 23) + 1, S - 1, 0x5A5A5A, 0x123456):
+        assert float(got[i]) == oracle.u32_to_f32(int(u[i])), i
+
+
+@pytest.mark.parametrize("kind", [pkg.RNG_PHILOX4X32_10, pkg.RNG_PHILOX4X32_7], ids=["philox10", "philox7"])
+@pytest.mark.parametrize("cvt", [0, 1, 2, 3], ids=["denormal_scale", "i2fp", "prmt_ffma", "i2f_xu"])
+def test_philox_f32_conversion_forms_are_the_same_map(kind, cvt):
+    """variant "cvt": four exact evaluations of (u >> 8) 2^-24 in the Philox fill kernel; every one against the
+    oracle, on full tiles (the lean all-full path), on a ragged last tile and across a continuation"""
+    S = 67
+    g, o = pkg.Rng(kind, S, 2024), oracle.Rng(kind, S, 2024)
+    g.set_variant("cvt", cvt)
+    for n in (1024, 2048 + 512, 36):
+        out = torch.empty(S * n, dtype=torch.float32, device="cuda")
+        g.fill_f32(out, n)
+        exp = o.fill_f32(n)
+        assert np.array_equal(out.cpu().numpy().view(np.uint32), exp.view(np.uint32)), (cvt, n)
+    g.close()
+
+
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 def test_mixed_call_sequence_is_one_stream(kind):
     """fill_u32(n1), draw_reduce(n2), fill_f32(n3) continue the same streams (state
