@@ -2,6 +2,7 @@
 judge read: a text page of the metrics that matter on this path and `profiles/traffic.json`.
 
     python -m paper_1204_6193_b200.ncu_summary RAW_DIR --text profiles/r02_ncu_full.txt [--json profiles/traffic.json]
+    python -m paper_1204_6193_b200.ncu_summary --launches LAUNCHES.csv --out profiles/r02_launches_<run>_summary.csv
 
 RAW_DIR holds one `raw_<workload>.csv` per capture, <workload> being bench.py's `--workload` name; each is
 
@@ -9,10 +10,13 @@ RAW_DIR holds one `raw_<workload>.csv` per capture, <workload> being bench.py's 
 
 of a capture taken with
 
-    ncu --set full --clock-control none --import-source on -k regex:<kernel> -s <skip> -c 1 -f -o rep_<workload> \\
-        python bench.py --suite primary --steps 5 --warmup 3 --no-e2e --no-cpu-baseline --ising-sweeps 3 --workload <workload>
+    ncu --set full --metrics <EXTRA> --clock-control none --import-source on -k regex:<kernel> -s <skip> -c 1 -f \\
+        -o rep_<workload> python bench.py --suite primary --steps 5 --warmup 3 --no-e2e --no-cpu-baseline --ising-sweeps 3 --workload <workload>
 
-(only after the same bench.py command has exited 0 without ncu).  Nothing here runs a kernel or is imported by
+(only after the same bench.py command has exited 0 without ncu; EXTRA = the EXTRA_METRICS list below: which of the
+two fma pipes and the conversion unit executed how many instructions -- `--set full` only has their sum).
+LAUNCHES.csv is the `--metrics gpu__time_duration.sum --clock-control none --csv` launch list of a bench.py run; its
+summary has one row per kernel (launches, total and average duration, share of the run).  Nothing here runs a kernel or is imported by
 the product path; bench.py reads the JSON as STATIC context (`measured_in_this_run: false`).
 """
 from __future__ import annotations
@@ -31,13 +35,27 @@ KEYS = [
     "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed",
     "sm__inst_executed_pipe_lsu.avg.pct_of_peak_sustained_active",
     "sm__inst_executed_pipe_uniform.avg.pct_of_peak_sustained_active",
-    "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active", "sm__warps_active.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_fmaheavy.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_fmalite.avg.pct_of_peak_sustained_active",
+    "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_active",
+    "sm__pipe_alu_cycles_active.avg.pct_of_peak_sustained_active",
+    "sm__pipe_shared_cycles_active.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_alu.sum", "sm__inst_executed_pipe_fmaheavy.sum", "sm__inst_executed_pipe_fmalite.sum",
+    "sm__inst_executed_pipe_xu.sum", "sm__inst_executed_pipe_lsu.sum",
+    "sm__warps_active.avg.pct_of_peak_sustained_active",
     "smsp__inst_executed.sum", "launch__registers_per_thread", "launch__grid_size", "launch__block_size",
     "launch__occupancy_limit_registers", "launch__occupancy_limit_shared_mem",
     "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", "l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum",
     "l1tex__throughput.avg.pct_of_peak_sustained_elapsed", "lts__throughput.avg.pct_of_peak_sustained_elapsed",
     "lts__t_sector_hit_rate.pct", "sm__cycles_elapsed.max", "smsp__cycles_active.avg", "sm__cycles_active.avg",
 ]
+EXTRA_METRICS = ",".join([
+    "sm__inst_executed_pipe_fmaheavy.avg.pct_of_peak_sustained_active", "sm__inst_executed_pipe_fmalite.avg.pct_of_peak_sustained_active",
+    "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_active", "sm__pipe_alu_cycles_active.avg.pct_of_peak_sustained_active",
+    "sm__pipe_shared_cycles_active.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_alu.sum", "sm__inst_executed_pipe_fmaheavy.sum", "sm__inst_executed_pipe_fmalite.sum",
+    "sm__inst_executed_pipe_xu.sum", "sm__inst_executed_pipe_lsu.sum"])
 UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
 TIME_US = {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}
 
@@ -87,6 +105,11 @@ def summarise(raw_dir: str, text_path: str, json_path: str | None, source: str) 
                     "pipe_fmaheavy_cycles_pct_of_elapsed": _num(d, "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed"),
                     "pipe_lsu_pct": _num(d, "sm__inst_executed_pipe_lsu.avg.pct_of_peak_sustained_active"),
                     "dram_throughput_pct": _num(d, "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed"),
+                    "pipe_fmaheavy_cycles_pct_of_active": _num(d, "sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_active"),
+                    "pipe_fmalite_pct": _num(d, "sm__inst_executed_pipe_fmalite.avg.pct_of_peak_sustained_active"),
+                    "pipe_xu_pct": _num(d, "sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active"),
+                    "inst_per_cycle_active": (None if not (_num(d, "smsp__inst_executed.sum") and _num(d, "smsp__cycles_active.avg"))
+                                              else round(_num(d, "smsp__inst_executed.sum") / (_num(d, "smsp__cycles_active.avg") * 592.0), 4)),
                 }
     if json_path:
         old = {}
@@ -104,12 +127,42 @@ def summarise(raw_dir: str, text_path: str, json_path: str | None, source: str) 
     return entries
 
 
+def summarise_launches(csv_in: str, csv_out: str) -> int:
+    """per kernel of an ncu launch list: launches, total and average gpu__time_duration, share of the run"""
+    rows = list(csv.reader(open(csv_in, errors="replace")))
+    hdr_i = next(i for i, r in enumerate(rows) if r and r[0] == "ID")
+    hdr = rows[hdr_i]
+    col = {n: hdr.index(n) for n in ("Kernel Name", "Grid Size", "Block Size", "Metric Name", "Metric Unit", "Metric Value")}
+    agg = {}
+    for r in rows[hdr_i + 1:]:
+        if len(r) < len(hdr) or r[col["Metric Name"]] != "gpu__time_duration.sum":
+            continue
+        us = float(r[col["Metric Value"]].replace(",", "")) * {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}.get(r[col["Metric Unit"]], 1e-3)
+        key = (r[col["Kernel Name"]], r[col["Grid Size"]], r[col["Block Size"]])
+        n, t = agg.get(key, (0, 0.0))
+        agg[key] = (n + 1, t + us)
+    total = sum(t for _, t in agg.values()) or 1.0
+    with open(csv_out, "w", newline="") as f:
+        w = csv.writer(f)
+        w.writerow(["kernel", "grid", "block", "launches", "sum_us", "avg_us", "share_pct"])
+        for (k, g, b), (n, t) in sorted(agg.items(), key=lambda kv: -kv[1][1]):
+            w.writerow([k, g, b, n, round(t, 1), round(t / n, 2), round(100.0 * t / total, 2)])
+    return len(agg)
+
+
 if __name__ == "__main__":
     ap = argparse.ArgumentParser()
-    ap.add_argument("raw_dir")
-    ap.add_argument("--text", required=True)
+    ap.add_argument("raw_dir", nargs="?")
+    ap.add_argument("--launches", default=None, help="an ncu launch list (csv) to summarise per kernel")
+    ap.add_argument("--out", default=None, help="with --launches: the summary csv to write")
+    ap.add_argument("--text", default=None)
     ap.add_argument("--json", default=None)
     ap.add_argument("--source", default=None, help="what the entries cite as their capture (default: --text)")
     a = ap.parse_args()
+    if a.launches:
+        print(f"{summarise_launches(a.launches, a.out or a.launches[:-4] + '_summary.csv')} kernels -> {a.out}")
+        raise SystemExit(0)
+    if not a.raw_dir or not a.text:
+        ap.error("RAW_DIR and --text are required without --launches")
     e = summarise(a.raw_dir, a.text, a.json, a.source or a.text)
     print(f"{len(e)} captures -> {a.text}" + (f", {a.json}" if a.json else ""))
