@@ -142,7 +142,7 @@ PAPER_GTX480 = {
 class ClockSampler:
     """samples SM clock and throttle reasons with NVML while the timed region runs"""
 
-    def __init__(self, index: int, period_s: float = 0.005):
+    def __init__(self, index: int, period_s: float = 0.001):
         self.index, self.period, self.samples, self.reasons = index, period_s, [], set()
         self._stop = threading.Event()
         self._thr = None
