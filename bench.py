@@ -3,6 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--suite primary|baseline|full]
     python bench.py --impl reference ...        # the CPU oracle on the host cores
+    python bench.py --fig1                      # the paper's Fig. 1 on this GPU (not a benchmark line)
 
 A "step" is one pass of the hot path over one batch of the named workload (seeded,
 synthetic -- this path has no dataset): for the default workload C2 (the config
@@ -654,6 +655,38 @@ def run_e2e(job: Job, steps: int, warmup: int, world: int) -> dict:
             if h2d == 0 else "lattice copied host->device and back every step"}
 
 
+def run_fig1(kinds=("lcg32", "lcg64", "xorwow", "philox4x32_10", "xs1024w", "lfib521"), n=4096, step=37, max_blocks=148 * 16):
+    """The analogue of the paper's Fig. 1: time per random number consumed in-register
+    (rng_draw_reduce, n draws per stream) as a function of the number of 256-stream blocks, which the paper
+    shows as a zig-zag commensurate with its 15 multiprocessors.  Returns {kind: [[blocks, ps_per_number], ...]}."""
+    import torch
+    import paper_1204_6193_b200 as pkg
+    by_name = {v: k for k, v in pkg.KIND_NAMES.items()}
+    out = {}
+    red = torch.empty(2 * 256 * max_blocks, dtype=torch.int32, device="cuda")
+    for name in kinds:
+        rows = []
+        for nb in range(step, max_blocks + 1, step):
+            S = 256 * nb
+            g = pkg.Rng(by_name[name], S, W.MASTER_SEED)
+            g.draw_reduce(red, n)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(3):
+                g.draw_reduce(red, n)
+            e1.record()
+            torch.cuda.synchronize()
+            g.close()
+            rows.append([nb, round(e0.elapsed_time(e1) / 3 * 1e9 / (S * n), 4)])  # picoseconds per number
+        out[name] = rows
+        best = min(r[1] for r in rows)
+        log(f"[fig1] {name}: best {best:.3f} ps per number = {1e3 / best:.0f} Gnum/s at "
+            f"{[r[0] for r in rows if r[1] == best][0]} blocks of 256 streams; "
+            + " ".join(f"{r[0]}:{r[1]:.2f}" for r in rows[:: max(1, len(rows) // 16)]))
+    return out
+
+
 SHORT_DESC = {
     "C2_u32": "Philox4x32-10, 2^20 streams x 1024 u32 = 4 GiB per step (BASELINE configs[1])",
     "C2_f32": "Philox4x32-10, 2^20 streams x 1024 f32 = 4 GiB per step (BASELINE configs[1], float variant)",
@@ -707,6 +740,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dump", default=None, help="also write every workload's full result as a JSON list to this file")
+    ap.add_argument("--fig1", action="store_true", help="instead of the benchmark: the paper's Fig. 1 on this GPU "
+                    "(time per in-register random number against the number of 256-stream blocks); JSON on stdout")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         log("[bench] note: timing rules ask for >= 3 warm-up steps")
@@ -731,6 +766,11 @@ def main():
         torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         torch.distributed.barrier()
     pkg.lib()
+    if args.fig1:
+        if rank == 0:
+            print(json.dumps({"fig1": run_fig1(), "unit": "ps per number", "x": "blocks of 256 streams, 4096 draws per stream",
+                              "cite": "PAPER.md:52"}), flush=True)
+        return 0
     suite = args.suite or ("baseline" if world == 1 and args.workload == "C2_u32" else "primary")
     buf = torch.empty(1 << 30, dtype=torch.int32, device="cuda")  # 4 GiB, reused by every workload (> L2)
 
