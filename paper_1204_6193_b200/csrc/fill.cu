@@ -525,7 +525,7 @@ cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, 
     case RNG_MWC: return launch_rowtile<RNG_MWC>(g, d_out, n, f32, h.var_store, st);
     case RNG_MWC_MULTI: return launch_rowtile<RNG_MWC_MULTI>(g, d_out, n, f32, h.var_store, st);
     case RNG_LFIB521:
-    case RNG_LFIB1279: return launch_lfib_fill(g, d_out, n, f32, st);
+    case RNG_LFIB1279: return launch_lfib_fill(g, d_out, n, f32, h.var_store, st);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -124,7 +124,7 @@ cudaError_t launch_seed(const Gen &g, LcgTable *tab, cudaStream_t st);
 cudaError_t launch_seed_mwc_multi(const Gen &g, cudaStream_t st);
 // lfib.cu (RNG_LFIB521 / RNG_LFIB1279: seeding and fill; draws and Ising go through Stream<KIND>)
 cudaError_t launch_seed_lfib(const Gen &g, cudaStream_t st);
-cudaError_t launch_lfib_fill(const Gen &g, void *d_out, uint64_t n, bool f32, cudaStream_t st);
+cudaError_t launch_lfib_fill(const Gen &g, void *d_out, uint64_t n, bool f32, int variant, cudaStream_t st);
 cudaError_t launch_lfib_draw(const Gen &g, uint32_t *d_out, uint64_t n, cudaStream_t st);
 // seed_xs1024_skip.cu (RNG_XS1024W_SKIP; synchronises the stream, frees its scratch)
 cudaError_t launch_seed_xs1024_skip(const Gen &g, cudaStream_t st);

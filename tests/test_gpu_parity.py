@@ -115,6 +115,26 @@ def test_philox_f32_conversion_forms_are_the_same_map(kind, cvt):
     g.close()
 
 
+@pytest.mark.parametrize("kind", LFIB_KINDS, ids=["lfib521", "lfib1279"])
+@pytest.mark.parametrize("store", [1, 2], ids=["tile32", "tile64"])
+def test_lfib_fill_tiles_ring_is_the_staging_buffer(kind, store):
+    """the lagged Fibonacci fill keeps 32 or 64 batches in its ring and writes rows out of it (lfib.cu): whole
+    tiles, several tiles, a ragged last tile, rows that are not 16-byte aligned, continuation across calls (the
+    state is reloaded into the last slots), u32 and f32, and the state at the end -- all against the oracle"""
+    S = 512
+    g, o = pkg.Rng(kind, S, 77), oracle.Rng(kind, S, 77)
+    g.set_variant("store", store)
+    for n in (64, 200, 32, 7, 1, 130, 3):
+        out = dev_u32(S * n)
+        g.fill_u32(out, n)
+        assert np.array_equal(host(out, S * n), o.fill_u32(n)), (store, n)
+        outf = torch.empty(max(S * n, 4), dtype=torch.float32, device="cuda")
+        g.fill_f32(outf, n)
+        assert np.array_equal(outf.cpu().numpy().view(np.uint32)[:S * n], o.fill_f32(n).view(np.uint32)), (store, n)
+        assert np.array_equal(g.get_state(), o.get_state()), (store, n)
+    g.close()
+
+
 @pytest.mark.parametrize("kind", KINDS, ids=IDS)
 def test_mixed_call_sequence_is_one_stream(kind):
     """fill_u32(n1), draw_reduce(n2), fill_f32(n3) continue the same streams (state
