@@ -431,7 +431,8 @@ static cudaError_t launch_rowtile(const Gen &g, void *d_out, uint64_t n, bool f3
 }
 
 template <bool F32, int U, int T, int R, int CVT = 0>
-static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uint64_t blocks_per_row, cudaStream_t st)
+static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uint64_t blocks_per_row, cudaStream_t st,
+                                      bool one_shot = false)
 {
     const uint64_t tpr = (blocks_per_row + 32 * U * T - 1) / (32 * U * T);
     const uint64_t n_tiles = g.S * tpr;
@@ -446,7 +447,7 @@ static cudaError_t launch_philox_warp(const Gen &g, uint32_t *o, uint64_t n, uin
     }
     uint64_t grid = (uint64_t)sm_count() * per_sm;
     const uint64_t need = (n_tiles + 7) / 8;
-    if (grid > need) grid = need;
+    if (grid > need || (one_shot && need <= 0x7fffffffull)) grid = need; // one_shot: one tile per warp, CTAs handed out by the hardware
     const uint64_t b0 = g.draws_done >> 2;
     // every tile full, and the call's blocks share the high counter word: the lean per-tile path
     const bool allfast = blocks_per_row % (32 * U * T) == 0 && (b0 >> 32) == ((b0 + blocks_per_row - 1) >> 32);
@@ -478,10 +479,17 @@ static cudaError_t launch_philox_fill(const Gen &g, void *d_out, uint64_t n, boo
             default: return launch_philox_warp<true, 8, 1, R, 3>(g, o, n, blocks_per_row, st);
             }
         }
+        // Grid: Philox4x32-10 is paced by its IMAD.WIDE arithmetic, every SM finishes its share at the same time and
+        // the persistent grid wins (624 us against 700 us per 4 GiB with one CTA per 8 tiles); the 7-round variant
+        // is store-bound, where a static split waits for the SMs that get the smaller share of the write bandwidth
+        // (DESIGN.md 6.4): one short-lived CTA per 8 tiles, handed out by the hardware, 690 -> 568 us = 7.56 TB/s.
+        // variant "store": 3 = one-shot CTAs, 4 = persistent grid, whatever R.
+        const bool one_shot = variant == 3 || (variant != 4 && R < 10);
         switch (variant) { // identical bits; (U, T) = blocks interleaved per lane, groups per tile
         case 1: return PW(4, 2);
         case 2: return PW(2, 4);
-        default: return PW(8, 1);
+        default: return f32 ? launch_philox_warp<true, 8, 1, R>(g, o, n, blocks_per_row, st, one_shot)
+                            : launch_philox_warp<false, 8, 1, R>(g, o, n, blocks_per_row, st, one_shot);
         }
 #undef PW
     }
