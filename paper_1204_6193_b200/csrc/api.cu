@@ -174,7 +174,7 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
         e = cudaMemsetAsync(h->ticket, 0, sizeof(uint64_t), 0);
     }
     if (e == cudaSuccess)
-        e = (kind == RNG_XS1024W_SKIP)                       ? launch_seed_xs1024_skip(h->g, 0)
+        e = (kind == RNG_XS1024W_SKIP)                       ? launch_seed_xs1024_skip(h->g, h->device, 0)
             : (kind == RNG_LFIB521 || kind == RNG_LFIB1279) ? launch_seed_lfib(h->g, 0)
             : (kind == RNG_MWC_MULTI)                       ? launch_seed_mwc_multi(h->g, 0)
                                                             : launch_seed(h->g, tab, 0);

@@ -127,7 +127,7 @@ cudaError_t launch_seed_lfib(const Gen &g, cudaStream_t st);
 cudaError_t launch_lfib_fill(const Gen &g, void *d_out, uint64_t n, bool f32, int variant, cudaStream_t st);
 cudaError_t launch_lfib_draw(const Gen &g, uint32_t *d_out, uint64_t n, cudaStream_t st);
 // seed_xs1024_skip.cu (RNG_XS1024W_SKIP; synchronises the stream, frees its scratch)
-cudaError_t launch_seed_xs1024_skip(const Gen &g, cudaStream_t st);
+cudaError_t launch_seed_xs1024_skip(const Gen &g, int device, cudaStream_t st);
 // fill.cu  (f32 = apply the (u>>8)*2^-24 map; out is uint32_t* or float*)
 cudaError_t launch_fill(const rng_handle &h, void *d_out, uint64_t n, bool f32, cudaStream_t st);
 // fill_xs1024.cu (XORShift1024/Weyl, K words per lane; variant "xs1024" = K, 64 = the generic kernels)

@@ -9,11 +9,14 @@
 //   2. J_0 = M^(2^137) by 137 squarings, J_k = J_{k-1}^2 = M^(2^(137+k));
 //   3. X(G0) = X_0 J^G0 for the shard's first instance G0, over the set bits of G0;
 //   4. level k: X(G0 + i + 2^k) = X(G0 + i) J_k for all i < 2^k at once.
-// Every instance costs ONE vector-matrix product however many instances there are.
+// Every instance costs ONE vector-matrix product however many instances there are.  Steps 1 and 2 do not depend on
+// the seed: their result is kept per device for the life of the process (xs_skip_matrices).
 // A matrix is uint32 [1024][32]: row r = image of the unit vector "word r/32, bit r%32"
 // (word 0 most significant, R-D1); a product X A is the XOR of the rows of A at the set bits of
 // X, with lane l of a warp holding word l of X and of the result.  128 KiB per matrix: L1/L2.
 // Product code (sm_100a); shares nothing with oracle/.
+#include <mutex>
+
 #include "internal.h"
 
 namespace rngb200 {
@@ -61,15 +64,18 @@ __global__ void __launch_bounds__(256) xs_matrix_square_kernel(uint32_t *__restr
 
 // step 3: one warp.  X_0 = the randomly seeded state of instance 0 (R-D7b: words 2k, 2k+1 =
 // lo32, hi32 of SM_seed[k], all-zero guard as in seed_xs1024_kernel); then X_0 J^G0.
-__global__ void __launch_bounds__(32) xs_skip_start_kernel(uint32_t *__restrict__ state, const uint32_t *__restrict__ Jall,
-                                                           uint64_t G0, uint64_t seed)
+struct XsSkipPtrs {
+    const uint32_t *J[64];
+};
+__global__ void __launch_bounds__(32) xs_skip_start_kernel(uint32_t *__restrict__ state, const XsSkipPtrs ptrs, uint64_t G0,
+                                                           uint64_t seed)
 {
     const int lane = threadIdx.x;
     const uint64_t z = splitmix64_at(seed, (uint64_t)(lane >> 1));
     uint32_t x = (lane & 1) ? (uint32_t)(z >> 32) : (uint32_t)z;
     if (!__any_sync(0xffffffffu, x != 0u) && lane == 31) x = 1u;
     for (int k = 0; k < 64 && (G0 >> k) != 0ull; k++)
-        if ((G0 >> k) & 1ull) x = xs_vecmat(x, Jall + (size_t)k * XS_MAT_WORDS, lane);
+        if ((G0 >> k) & 1ull) x = xs_vecmat(x, ptrs.J[k], lane);
     state[lane] = x;
 }
 
@@ -83,31 +89,73 @@ __global__ void __launch_bounds__(256) xs_skip_level_kernel(uint32_t *__restrict
     state[(have + i) * 32 + lane] = xs_vecmat(state[i * 32 + lane], Jk, lane);
 }
 
-cudaError_t launch_seed_xs1024_skip(const Gen &g, cudaStream_t st)
+// The skip matrices J_k = M^(2^(137+k)) depend on the generator only, not on the seed or the handle: they are
+// computed once per device and process (the paper ships its matrix in a header; 128 KiB per level here, 2.5 MiB for
+// 2^19 instances) and extended when a later handle needs more levels.  Complete levels are immutable, and the stream
+// that computed them was synchronised before `levels` was raised, so any later stream may read them.
+struct XsSkipCache {
+    uint32_t *J[64] = {};
+    int levels = 0;
+};
+static std::mutex g_xs_skip_mutex;
+static XsSkipCache g_xs_skip_cache[64]; // by device ordinal
+
+// makes J_0 .. J_{levels-1} of `device` available; *launched = kernels launched for it
+static cudaError_t xs_skip_matrices(int device, int levels, cudaStream_t st, uint32_t *const **J, uint64_t *launched)
+{
+    *launched = 0;
+    if (device < 0 || device >= 64 || levels > 64) return cudaErrorInvalidValue;
+    std::lock_guard<std::mutex> lock(g_xs_skip_mutex);
+    XsSkipCache &c = g_xs_skip_cache[device];
+    *J = c.J;
+    if (c.levels >= levels) return cudaSuccess;
+    cudaError_t e = cudaSuccess;
+    for (int k = c.levels; k < levels && e == cudaSuccess; k++)
+        if (!c.J[k]) e = cudaMalloc((void **)&c.J[k], (size_t)XS_MAT_WORDS * 4);
+    if (e != cudaSuccess) return e;
+    if (c.levels == 0) {
+        uint32_t *tmp = nullptr;
+        e = cudaMalloc((void **)&tmp, (size_t)2 * XS_MAT_WORDS * 4);
+        if (e != cudaSuccess) return e;
+        uint32_t *a = tmp, *b = tmp + XS_MAT_WORDS;
+        xs_unit_matrix_kernel<<<128, 256, 0, st>>>(a);
+        for (int i = 0; i < 137; i++) { // M^(2^137): the sub-stream length of PAPER.md:228
+            xs_matrix_square_kernel<<<128, 256, 0, st>>>(i == 136 ? c.J[0] : b, a);
+            uint32_t *t = a;
+            a = b;
+            b = t;
+        }
+        *launched += 138;
+        e = cudaStreamSynchronize(st);
+        cudaFree(tmp);
+        if (e != cudaSuccess) return e;
+        c.levels = 1;
+    }
+    for (int k = c.levels; k < levels; k++) {
+        xs_matrix_square_kernel<<<128, 256, 0, st>>>(c.J[k], c.J[k - 1]);
+        (*launched)++;
+    }
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) c.levels = levels;
+    return e;
+}
+
+cudaError_t launch_seed_xs1024_skip(const Gen &g, int device, cudaStream_t st)
 {
     const uint64_t n_inst = g.S / 32, G0 = g.first / 32;
     int levels = 0; // matrices J_0 .. J_{levels-1}
     while (levels < 64 && (((G0 >> levels) != 0ull) || ((1ull << levels) < n_inst))) levels++;
     if (levels < 1) levels = 1;
-    uint32_t *Jall = nullptr, *tmp = nullptr;
-    cudaError_t e = cudaMalloc((void **)&Jall, (size_t)levels * XS_MAT_WORDS * 4);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&tmp, (size_t)2 * XS_MAT_WORDS * 4);
-    if (e != cudaSuccess) {
-        cudaFree(Jall);
-        return e;
-    }
-    uint32_t *a = tmp, *b = tmp + XS_MAT_WORDS;
-    xs_unit_matrix_kernel<<<128, 256, 0, st>>>(a);
-    for (int i = 0; i < 137; i++) { // M^(2^137): the sub-stream length of PAPER.md:228
-        xs_matrix_square_kernel<<<128, 256, 0, st>>>(i == 136 ? Jall : b, a);
-        uint32_t *t = a;
-        a = b;
-        b = t;
-    }
-    for (int k = 1; k < levels; k++)
-        xs_matrix_square_kernel<<<128, 256, 0, st>>>(Jall + (size_t)k * XS_MAT_WORDS, Jall + (size_t)(k - 1) * XS_MAT_WORDS);
-    xs_skip_start_kernel<<<1, 32, 0, st>>>((uint32_t *)g.state, Jall, G0, g.seed);
-    uint64_t launches = 1 + 137 + (uint64_t)(levels - 1) + 1;
+    uint32_t *const *J = nullptr;
+    uint64_t launches = 0;
+    cudaError_t e = xs_skip_matrices(device, levels, st, &J, &launches);
+    if (e != cudaSuccess) return e;
+    // the start kernel walks the set bits of G0 through a table of the levels' pointers
+    XsSkipPtrs ptrs;
+    for (int k = 0; k < 64; k++) ptrs.J[k] = k < levels ? J[k] : nullptr;
+    xs_skip_start_kernel<<<1, 32, 0, st>>>((uint32_t *)g.state, ptrs, G0, g.seed);
+    launches++;
     int k = 0;
     for (uint64_t have = 1; have < n_inst; have <<= 1, k++) {
         const uint64_t warps = (n_inst - have < have) ? (n_inst - have) : have;
@@ -116,15 +164,12 @@ cudaError_t launch_seed_xs1024_skip(const Gen &g, cudaStream_t st)
             e = cudaErrorInvalidConfiguration;
             break;
         }
-        xs_skip_level_kernel<<<(unsigned)grid, 256, 0, st>>>((uint32_t *)g.state, Jall + (size_t)k * XS_MAT_WORDS, have, n_inst);
+        xs_skip_level_kernel<<<(unsigned)grid, 256, 0, st>>>((uint32_t *)g.state, J[k], have, n_inst);
         launches++;
     }
     count_launch(launches);
     if (e == cudaSuccess) e = cudaGetLastError();
-    const cudaError_t es = cudaStreamSynchronize(st); // the matrices must outlive the kernels that read them
-    cudaFree(Jall);
-    cudaFree(tmp);
-    return e != cudaSuccess ? e : es;
+    return e;
 }
 
 } // namespace rngb200
