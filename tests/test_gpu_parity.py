@@ -115,6 +115,25 @@ def test_philox_f32_conversion_forms_are_the_same_map(kind, cvt):
     g.close()
 
 
+@pytest.mark.parametrize("kind", [pkg.RNG_PHILOX4X32_10, pkg.RNG_PHILOX4X32_7], ids=["philox10", "philox7"])
+@pytest.mark.parametrize("store", [1, 2, 3, 4], ids=["U4T2", "U2T4", "one_shot_ctas", "persistent_grid"])
+def test_philox_fill_grid_and_tile_variants(kind, store):
+    """variant "store" of the Philox fill: blocks per lane x groups per tile, and who hands out the tiles (a
+    persistent grid striding over them, or one short-lived CTA per 8 tiles); full tiles, more tiles than one wave
+    of CTAs, a ragged last tile, continuation, u32 and f32 -- all against the oracle"""
+    S = 3000  # x 3 tiles per row for n = 3072: 9000 tiles = 1125 one-shot CTAs
+    g, o = pkg.Rng(kind, S, 31), oracle.Rng(kind, S, 31)
+    g.set_variant("store", store)
+    for n in (3072, 1024, 520):
+        out = dev_u32(S * n)
+        g.fill_u32(out, n)
+        assert np.array_equal(host(out, S * n), o.fill_u32(n)), (store, n)
+        outf = torch.empty(S * n, dtype=torch.float32, device="cuda")
+        g.fill_f32(outf, n)
+        assert np.array_equal(outf.cpu().numpy().view(np.uint32), o.fill_f32(n).view(np.uint32)), (store, n)
+    g.close()
+
+
 @pytest.mark.parametrize("kind", LFIB_KINDS, ids=["lfib521", "lfib1279"])
 @pytest.mark.parametrize("store", [1, 2], ids=["tile32", "tile64"])
 def test_lfib_fill_tiles_ring_is_the_staging_buffer(kind, store):
