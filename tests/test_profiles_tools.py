@@ -1,0 +1,37 @@
+"""-m "not gpu": the committed profile summaries are what the committed tools make of the committed raw lists
+(host logic only; nothing here runs a kernel)."""
+import csv
+import json
+import os
+
+from paper_1204_6193_b200 import ncu_summary
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+PROF = os.path.join(ROOT, "profiles")
+
+
+def test_launch_summary_is_reproducible_from_the_raw_launch_list(tmp_path):
+    raw = os.path.join(PROF, "r02_launches_bench_primary.csv")
+    out = tmp_path / "summary.csv"
+    n = ncu_summary.summarise_launches(raw, str(out))
+    got = list(csv.reader(open(out)))
+    exp = list(csv.reader(open(os.path.join(PROF, "r02_launches_bench_primary_summary.csv"))))
+    assert n == len(got) - 1 and got == exp
+    # the headline kernel is every launch of the library in the primary step
+    lib = [r for r in got[1:] if "rngb200::" in r[0]]
+    assert len(lib) == 1 and "philox_fill_warp_kernel" in lib[0][0] and int(lib[0][3]) == 23  # 20 steps + 3 warm-up
+
+
+def test_traffic_json_entries_cite_existing_captures_and_carry_the_bench_keys():
+    d = json.load(open(os.path.join(PROF, "traffic.json")))
+    entries = {k: v for k, v in d.items() if not k.startswith("_")}
+    assert {"C2_u32", "C2_f32", "C3_draw", "C4_fill", "C4_draw", "C5b_philox", "C5b_xorwow"} <= set(entries)
+    for name, e in entries.items():
+        assert os.path.exists(os.path.join(ROOT, e["source"])), (name, e["source"])
+        text = open(os.path.join(ROOT, e["source"])).read()
+        kernel = e["kernel"].replace("void ", "").split("(")[0]
+        assert kernel in text, (name, kernel)  # the capture the entry cites holds this kernel
+        for key in ("kernel", "dram_bytes_per_launch", "ncu_time_us", "issue_active_pct"):
+            assert key in e, (name, key)
+    # algorithmic bytes of the headline (4 B x 2^30 draws) against the measured DRAM traffic: no wasted re-reads
+    assert 0.95 < entries["C2_u32"]["dram_bytes_per_launch"] / (4 * 2 ** 30) < 1.02
