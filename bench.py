@@ -340,6 +340,17 @@ class IsingJob(Job):
         self.rng.close()
 
 
+def max_over_ranks(ms: float) -> float:
+    """the slowest rank's time (the contract's max over ranks); the tensor lives where the backend reduces: on
+    the GPU for nccl, on the host for gloo (the CPU-side rendezvous test of the N > 1 flow)"""
+    import torch
+    dist = torch.distributed
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def roofline(name: str, bound: str, alg_per_launch: float, sec_per_launch: float, store_gbs=None) -> dict:
     """the `roofline` object of one workload.  hbm: algorithmic bytes per launch / measured launch duration against
     the measured copy bandwidth (MEASURED_PEAKS.json), and against the live write-only (memset) ceiling of this run
@@ -396,9 +407,7 @@ def run_job(job: Job, steps: int, warmup: int, world: int, sample_clocks: bool, 
     launches = pkg.rng_kernel_launches() - l0
     ms = ev0.elapsed_time(ev1)
     if dist:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+        ms = max_over_ranks(ms)
         dist.barrier()
     units = job.units_per_step() * steps * world
     per_s = units / (ms * 1e-3)
@@ -645,9 +654,7 @@ def run_e2e(job: Job, steps: int, warmup: int, world: int) -> dict:
     wall_ms = (time.perf_counter() - t0) * 1e3
     ms = max(ev0.elapsed_time(ev1), wall_ms)  # the host call blocks: wall clock is the honest one
     if dist:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+        ms = max_over_ranks(ms)
     val = job.units_per_step() * steps * world / (ms * 1e-3) / 1e9
     return {"value": val, "unit": job.unit, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": steps,
             "ms_per_step": ms / steps, "api": api,
@@ -740,6 +747,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dump", default=None, help="also write every workload's full result as a JSON list to this file")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="torch.distributed backend for N > 1 (nccl: one rank per GPU; gloo only for flow tests)")
     ap.add_argument("--fig1", action="store_true", help="instead of the benchmark: the paper's Fig. 1 on this GPU "
                     "(time per in-register random number against the number of 256-stream blocks); JSON on stdout")
     args = ap.parse_args()
@@ -761,9 +770,13 @@ def main():
         pkg_build.build()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
+    dev_index = local_rank % torch.cuda.device_count()  # == local_rank with one rank per GPU
+    torch.cuda.set_device(dev_index)
     if world > 1:
-        torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if args.dist_backend == "nccl":
+            torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", dev_index))
+        else:  # gloo: only to exercise the N > 1 flow where ranks must share a GPU (tests); timings mean nothing
+            torch.distributed.init_process_group(args.dist_backend)
         torch.distributed.barrier()
     pkg.lib()
     if args.fig1:
@@ -779,7 +792,7 @@ def main():
     store_gbs = ceil["memset_write_gbs"]
 
     job = make_job(args.workload, rank, world, buf, args.ising_sweeps)
-    res = run_job(job, args.steps, args.warmup, world, sample_clocks=True, dev_index=local_rank, store_gbs=store_gbs)
+    res = run_job(job, args.steps, args.warmup, world, sample_clocks=True, dev_index=dev_index, store_gbs=store_gbs)
     e2e = None if args.no_e2e else run_e2e(job, args.e2e_steps, 1, world)
     cfg_info = {"desc": SHORT_DESC.get(args.workload, res["name"]),
                 "streams_per_gpu": getattr(getattr(job, "cfg", None), "n_streams", getattr(job, "n_local", None)),
@@ -800,7 +813,7 @@ def main():
         if name == args.workload:
             continue
         j = make_job(name, rank, world, buf, args.ising_sweeps)
-        r = run_job(j, k, w, world, sample_clocks=False, dev_index=local_rank, store_gbs=store_gbs)
+        r = run_job(j, k, w, world, sample_clocks=False, dev_index=dev_index, store_gbs=store_gbs)
         j.close()
         r["workload"] = name
         configs.append(r)
