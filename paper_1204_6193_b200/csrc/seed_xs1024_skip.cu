@@ -89,6 +89,50 @@ __global__ void __launch_bounds__(256) xs_skip_level_kernel(uint32_t *__restrict
     state[(have + i) * 32 + lane] = xs_vecmat(state[i * 32 + lane], Jk, lane);
 }
 
+// ---- large levels: the product through byte tables ("four Russians") ----
+// For a level with many instances the rows of J_k are first combined into a table T[c][v] = XOR of the rows
+// 8c + b over the set bits b of the byte value v (c = 0..127, v = 0..255; 4 MiB, L2-resident): a product is then 128
+// table rows instead of one predicated row load for each of the 1024 bits -- a sixth of the instructions.
+// Byte c of X = byte c % 4 of word c / 4; bit b of that byte is bit 8 (c % 4) + b of the word, i.e. row
+// 32 (c / 4) + 8 (c % 4) + b = 8c + b of the matrix.
+constexpr int XS_TAB_WORDS = 128 * 256 * 32;
+
+// one CTA per table position c: generation j doubles the table, entry v in [2^j, 2^(j+1)) = entry v - 2^j ^ row 8c + j
+__global__ void __launch_bounds__(256) xs_byte_table_kernel(uint32_t *__restrict__ T, const uint32_t *__restrict__ J)
+{
+    __shared__ uint32_t tab[256 * 32];
+    const int c = (int)blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (warp == 0) tab[lane] = 0u;
+    __syncthreads();
+    for (int j = 0; j < 8; j++) {
+        const uint32_t row = J[(8 * c + j) * 32 + lane];
+        for (int v = (1 << j) + warp; v < (2 << j); v += 8) tab[v * 32 + lane] = tab[(v - (1 << j)) * 32 + lane] ^ row;
+        __syncthreads();
+    }
+    uint32_t *t = T + (size_t)c * 256 * 32;
+    for (int i = threadIdx.x; i < 256 * 32; i += 256) t[i] = tab[i];
+}
+
+__global__ void __launch_bounds__(256) xs_skip_level_table_kernel(uint32_t *__restrict__ state, const uint32_t *__restrict__ T,
+                                                                  uint64_t have, uint64_t n_inst)
+{
+    const uint64_t i = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (i >= have || have + i >= n_inst) return; // warp-uniform
+    const uint32_t xw = state[i * 32 + lane];
+    uint32_t acc0 = 0u, acc1 = 0u, acc2 = 0u, acc3 = 0u;
+#pragma unroll 4
+    for (int w = 0; w < 32; w++) {
+        const uint32_t xv = __shfl_sync(0xffffffffu, xw, w); // warp-uniform word w of X
+        const uint32_t *t = T + (size_t)(4 * w) * 256 * 32 + lane;
+        acc0 ^= t[(size_t)(xv & 255u) * 32];
+        acc1 ^= t[(size_t)(256 + ((xv >> 8) & 255u)) * 32];
+        acc2 ^= t[(size_t)(512 + ((xv >> 16) & 255u)) * 32];
+        acc3 ^= t[(size_t)(768 + (xv >> 24)) * 32];
+    }
+    state[(have + i) * 32 + lane] = (acc0 ^ acc1) ^ (acc2 ^ acc3);
+}
+
 // The skip matrices J_k = M^(2^(137+k)) depend on the generator only, not on the seed or the handle: they are
 // computed once per device and process (the paper ships its matrix in a header; 128 KiB per level here, 2.5 MiB for
 // 2^19 instances) and extended when a later handle needs more levels.  Complete levels are immutable, and the stream
@@ -157,6 +201,8 @@ cudaError_t launch_seed_xs1024_skip(const Gen &g, int device, cudaStream_t st)
     xs_skip_start_kernel<<<1, 32, 0, st>>>((uint32_t *)g.state, ptrs, G0, g.seed);
     launches++;
     int k = 0;
+    uint32_t *table = nullptr; // byte table of the current level (levels of at least kTableFrom instances)
+    constexpr uint64_t kTableFrom = 4096;
     for (uint64_t have = 1; have < n_inst; have <<= 1, k++) {
         const uint64_t warps = (n_inst - have < have) ? (n_inst - have) : have;
         const uint64_t grid = (warps * 32 + 255) / 256;
@@ -164,11 +210,24 @@ cudaError_t launch_seed_xs1024_skip(const Gen &g, int device, cudaStream_t st)
             e = cudaErrorInvalidConfiguration;
             break;
         }
-        xs_skip_level_kernel<<<(unsigned)grid, 256, 0, st>>>((uint32_t *)g.state, J[k], have, n_inst);
-        launches++;
+        if (warps >= kTableFrom) {
+            if (!table) e = cudaMalloc((void **)&table, (size_t)XS_TAB_WORDS * 4);
+            if (e != cudaSuccess) break;
+            xs_byte_table_kernel<<<128, 256, 0, st>>>(table, J[k]); // stream order: after the previous level's reads
+            xs_skip_level_table_kernel<<<(unsigned)grid, 256, 0, st>>>((uint32_t *)g.state, table, have, n_inst);
+            launches += 2;
+        } else {
+            xs_skip_level_kernel<<<(unsigned)grid, 256, 0, st>>>((uint32_t *)g.state, J[k], have, n_inst);
+            launches++;
+        }
     }
     count_launch(launches);
     if (e == cudaSuccess) e = cudaGetLastError();
+    if (table) { // the table must outlive the kernels that read it
+        const cudaError_t es = cudaStreamSynchronize(st);
+        cudaFree(table);
+        if (e == cudaSuccess) e = es;
+    }
     return e;
 }
 
