@@ -210,6 +210,38 @@ int ising_sweep(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_
 int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta, uint32_t n_sweeps,
                          uint32_t tile, uint32_t k_hits, int64_t *d_energy_trace, void *cuda_stream);
 
+/* ---- a8 without allocation: for callers that cannot call cudaMalloc ---------------
+ * ising_sweep needs a handle (rng_create allocates) and, on its multi-spin path, allocates the
+ * two bit planes it works on.  That shuts out callers who cannot obtain device memory when they
+ * want to sweep: a simulation sharing the GPU with a framework whose caching allocator already
+ * holds all of HBM, a latency-critical loop that cannot take the device-wide synchronisation
+ * cudaMalloc/cudaFree imply, a process whose memory budget was fixed when it started.  This entry
+ * point serves them.  It calls no cudaMalloc, cudaFree or allocating library routine, ever:
+ *  - the generator is Philox4x32-10 (kind 3), which stores no state, so there is no handle; the
+ *    caller carries the stream position: pass draws_done (a multiple of 4; 0 for fresh streams) and
+ *    pass draws_done + 2*K*n_sweeps to the next call, K = (L*L/2)/n_streams;
+ *  - the bit planes live in a fixed array inside the library image (RNG_ISING_STATIC_MAX_L^2/8 =
+ *    2 MiB).  Every GPU that loads the library holds that array until the process exits, used or
+ *    not.  L > RNG_ISING_STATIC_MAX_L is refused with RNG_E_INVAL (the scratch never grows).
+ * Result: d_spins (and d_energy_trace) are bit-identical to ising_sweep on a handle from
+ * rng_create(RNG_PHILOX4X32_10, n_streams, seed) whose draws_done is the value passed here;
+ * site numbering, acceptance rule and trace are ising_sweep's (see above).  Only the multi-spin
+ * geometries are served: L a multiple of 64, 64 <= L <= RNG_ISING_STATIC_MAX_L; n_streams divides
+ * L*L/2 with K = 4, 8, 16 or a multiple of 32; beta >= 0 (else RNG_E_INVAL / RNG_E_UNSUPPORTED).
+ * Things to know:
+ *  - the first call on each device looks up the array's device address (once per device, with
+ *    that device current) and may make the runtime load the library's kernels there; make that
+ *    first call during set-up, before any stream capture.  n_sweeps = 1 on a scratch lattice will do.
+ *  - all calls on one device share the one array, and it keeps what the last call left.  Nothing
+ *    in it has to start at zero (each call rewrites every word it later reads), but two calls that
+ *    overlap on the GPU -- different streams, or different host threads -- race on it and corrupt
+ *    each other's lattices.  Issue them on one stream, or order them yourself.
+ *  - d_spins / d_energy_trace are the caller's device buffers, as for ising_sweep; the call only
+ *    enqueues work.  After RNG_E_CUDA the lattice contents are unspecified. */
+#define RNG_ISING_STATIC_MAX_L 4096u
+int ising_sweep_philox_static(uint64_t n_streams, uint64_t seed, uint64_t draws_done, int8_t *d_spins, uint32_t L,
+                              double beta, uint32_t n_sweeps, int64_t *d_energy_trace, void *cuda_stream);
+
 /* helpers (not hot path) */
 /* spin i = +1 if bit (i & 63) of SM_seed[i >> 6] is set, else -1 */
 int ising_init_random(int8_t *d_spins, uint32_t L, uint64_t seed, void *cuda_stream);

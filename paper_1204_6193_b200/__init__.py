@@ -11,7 +11,7 @@ from .binding import (  # noqa: F401
     RNG_OK, RNG_E_INVAL, RNG_E_NOMEM, RNG_E_CUDA, RNG_E_UNSUPPORTED,
     KIND_NAMES, RngError, Rng, lib, library_path, EXPORTS,
     rng_create, rng_create_shard, rng_destroy, rng_fill_u32, rng_fill_f32, rng_draw_reduce,
-    ising_sweep, ising_sweep_multihit, ising_init_random, ising_energy, ising_accept_table,
+    ising_sweep, ising_sweep_multihit, ising_sweep_philox_static, RNG_ISING_STATIC_MAX_L, ising_init_random, ising_energy, ising_accept_table,
     rng_fill_u32_host, rng_fill_f32_host, rng_draw_reduce_host, ising_sweep_host,
     rng_state_bytes, rng_get_state, rng_set_state, rng_draws_done, rng_set_draws_done,
     rng_set_variant, rng_kernel_launches, rng_last_error, rng_version,

@@ -34,6 +34,7 @@ EXPORTS = {
     "rng_draw_reduce": (_i32, [_vp, _vp, _u64, _vp]),
     "ising_sweep": (_i32, [_vp, _vp, _u32, _dbl, _u32, _vp, _vp]),
     "ising_sweep_multihit": (_i32, [_vp, _vp, _u32, _dbl, _u32, _u32, _u32, _vp, _vp]),
+    "ising_sweep_philox_static": (_i32, [_u64, _u64, _u64, _vp, _u32, _dbl, _u32, _vp, _vp]),
     "ising_init_random": (_i32, [_vp, _u32, _u64, _vp]),
     "ising_energy": (_i32, [_vp, _u32, _vp, _vp]),
     "ising_accept_table": (_i32, [_dbl, _vp, _vp]),
@@ -155,6 +156,18 @@ def ising_sweep_multihit(h, d_spins, L: int, beta: float, n_sweeps: int, tile: i
                          cuda_stream=None) -> None:
     _check(lib().ising_sweep_multihit(h, _ptr(d_spins), L, float(beta), n_sweeps, tile, k_hits, _ptr(d_energy_trace),
                                       _stream(cuda_stream)))
+
+
+RNG_ISING_STATIC_MAX_L = 4096
+
+
+def ising_sweep_philox_static(n_streams: int, seed: int, draws_done: int, d_spins, L: int, beta: float, n_sweeps: int,
+                              d_energy_trace=None, cuda_stream=None) -> None:
+    """ising_sweep for callers that cannot allocate device memory (no handle, Philox4x32-10, the bit planes in
+    a fixed 2 MiB array of the library: L <= RNG_ISING_STATIC_MAX_L).  The caller keeps the stream position:
+    the next call takes draws_done + n_sweeps * L * L // n_streams.  See include/rng_b200.h."""
+    _check(lib().ising_sweep_philox_static(n_streams, seed & (2**64 - 1), draws_done, _ptr(d_spins), L, float(beta), n_sweeps,
+                                           _ptr(d_energy_trace), _stream(cuda_stream)))
 
 
 def ising_init_random(d_spins, L: int, seed: int, cuda_stream=None) -> None:

@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "librng_b200.so")
-SOURCES = ["seed.cu", "seed_xs1024_skip.cu", "lfib.cu", "mwc_multi.cu", "fill.cu", "fill_xs1024.cu", "draw.cu", "ising.cu", "ising_ms.cu", "ising_mh.cu", "api.cu"]
+SOURCES = ["seed.cu", "seed_xs1024_skip.cu", "lfib.cu", "mwc_multi.cu", "fill.cu", "fill_xs1024.cu", "draw.cu", "ising.cu", "ising_ms.cu", "ising_mh.cu", "ising_static.cu", "api.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC,-Wall,-Wno-unused-function", "-DRNG_B200",

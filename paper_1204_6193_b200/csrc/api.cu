@@ -56,6 +56,15 @@ int ensure_staging(rng_handle *h, uint64_t bytes)
 
 namespace rngb200 {
 void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+// for entry points that live in other files: leaves the message where rng_last_error() finds it, returns `code`
+int report_error(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
 int sm_count(int device)
 {
     static std::atomic<int> cache[64];

@@ -115,6 +115,8 @@ __device__ __forceinline__ void pdl_entry()
 #endif
 
 void count_launch(uint64_t n = 1);
+// sets the calling thread's rng_last_error() message and returns `code` (for entry points outside api.cu)
+int report_error(int code, const char *fmt, ...);
 // number of SMs of `device` (cached per device; 148 on a B200)
 int sm_count(int device);
 
