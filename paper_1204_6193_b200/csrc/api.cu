@@ -179,7 +179,6 @@ int rng_create_shard(int kind, uint64_t n_total, uint64_t first, uint64_t n_loca
     if (e == cudaSuccess) e = cudaMalloc(&h->energy_scratch, 2 * sizeof(int64_t));
     if (e == cudaSuccess) {
         h->ticket = (uint64_t *)(h->energy_scratch + 1);
-        h->ticket_base = 0;
         e = cudaMemsetAsync(h->ticket, 0, sizeof(uint64_t), 0);
     }
     if (e == cudaSuccess)
@@ -355,9 +354,16 @@ int ising_sweep_multihit(rng_handle *h, int8_t *d_spins, uint32_t L, double beta
             CU(cudaMalloc((void **)&h->mh_mailbox, need));
             h->mh_mailbox_bytes = need;
         }
-        CU(launch_ising_multihit_coop(*h, d_spins, L, tab, tile, k_hits, n_sweeps, d, h->mh_mailbox, st));
-        h->g.draws_done = d + per_sweep * n_sweeps;
-        return RNG_OK;
+        const cudaError_t ce = launch_ising_multihit_coop(*h, d_spins, L, tab, tile, k_hits, n_sweeps, d, h->mh_mailbox, st);
+        if (ce == cudaSuccess) {
+            h->g.draws_done = d + per_sweep * n_sweeps;
+            return RNG_OK;
+        }
+        // The one launch was refused (not every CTA can be resident: MPS or partition limits, fewer SMs than planned).
+        // Nothing of it ran -- the zeroed mailbox is harmless -- so in automatic mode the call is served by the
+        // per-colour launches below, as it was before the one-launch path existed; only variant 4 (forced) reports it.
+        if (h->var_ising == 4) return cuda_fail(ce, "launch_ising_multihit_coop");
+        cudaGetLastError();
     }
     for (uint32_t t = 0; t < n_sweeps; t++) {
         for (int c = 0; c < 2; c++) {

@@ -18,6 +18,8 @@
 //   columns of Table 1 are this kernel with k_hits = 1 and 100.
 // Acceptance as everywhere: flip iff (r >> 8) < T[(h+4)/2]  (exactly (float)(r>>8) 2^-24 < P).
 // Product code (sm_100a); shares nothing with oracle/.
+#include <atomic>
+
 #include "internal.h"
 #include "streams.cuh"
 
@@ -315,10 +317,29 @@ struct MhCoop {
     uint32_t slots, rounds, grid, threads;
     size_t smem;
 };
+// does `device` accept cooperative launches at all (cached per device; false when the query fails)
+static bool coop_launch_supported(int device)
+{
+    static std::atomic<int> cache[64]; // 0 = not asked, 1 = no, 2 = yes
+    if (device < 0 || device >= 64) return false;
+    int v = cache[device].load(std::memory_order_relaxed);
+    if (v == 0) {
+        int ok = 0;
+        if (cudaDeviceGetAttribute(&ok, cudaDevAttrCooperativeLaunch, device) != cudaSuccess) {
+            cudaGetLastError();
+            ok = 0;
+        }
+        v = ok ? 2 : 1;
+        cache[device].store(v, std::memory_order_relaxed);
+    }
+    return v == 2;
+}
+
 static MhCoop mh_coop_plan(const rng_handle &h, uint32_t L, uint32_t T, uint32_t n_sweeps)
 {
     MhCoop c{0u, 0u, 0u, 0u, 0};
     const uint32_t tile_threads = T * T / 2u;
+    if (!coop_launch_supported(h.device)) return c;       // e.g. some MPS / partitioned set-ups: per-colour launches
     if (kind_is_lfib(h.g.kind)) return c;                 // ring shared by a 256-thread CTA: its own CTA shape
     if (tile_threads % 32u || tile_threads > 1024u || T > 44u) return c; // named barriers count whole warps
     if (2ull * n_sweeps >= (1ull << kMhEpochBits)) return c;
@@ -388,9 +409,16 @@ cudaError_t launch_ising_multihit_coop(const rng_handle &h, int8_t *d_spins, uin
         e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
         if (e != cudaSuccess) return e;
     }
+    // every CTA must be resident at once (the tiles wait for their neighbours' halos): ask the occupancy
+    // calculator, not the SM count alone -- fewer SMs (MPS, partitions) or spills would make the launch too large
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, (int)c.threads, c.smem);
+    if (e != cudaSuccess) return e;
+    if ((uint64_t)per_sm * (uint64_t)sm_count(h.device) < c.grid) return cudaErrorCooperativeLaunchTooLarge;
     e = cudaLaunchCooperativeKernel(fn, dim3(c.grid), dim3(c.threads), args, c.smem, st);
+    if (e != cudaSuccess) return e; // refused: nothing ran (the caller may fall back to per-colour launches)
     count_launch();
-    return e != cudaSuccess ? e : cudaGetLastError();
+    return cudaGetLastError();
 }
 
 cudaError_t launch_ising_multihit(const rng_handle &h, int8_t *d_spins, uint32_t L, const IsingTable &tab, uint32_t T,

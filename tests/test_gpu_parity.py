@@ -707,6 +707,37 @@ def test_ising_multihit_whole_call_in_one_launch_bit_exact(kind, L, T, k, sweeps
     g2.close()
 
 
+@pytest.mark.parametrize("kind", [pkg.RNG_XORWOW, pkg.RNG_PHILOX4X32_10, pkg.RNG_XS1024W, pkg.RNG_LCG64, pkg.RNG_MWC_MULTI],
+                         ids=["xorwow", "philox10", "xs1024w", "lcg64", "mwc_multi"])
+@pytest.mark.parametrize("L,T,k,sweeps,one_launch", [(96, 24, 2, 3, True), (160, 40, 1, 3, True), (80, 40, 3, 2, True),
+                                                     (240, 40, 2, 2, True), (176, 44, 2, 2, False), (72, 36, 1, 2, False)])
+def test_ising_multihit_one_launch_wide_and_odd_tiles(kind, L, T, k, sweeps, one_launch):
+    """tiles wider than 32 sites (the second ballot of a halo row, spin bits 32..43 of the 64-bit mailbox word beside
+    its 20-bit stage number) and tile shapes whose CTA holds a number of tiles that is not a power of two (T = 24:
+    three tiles, 864 threads, named barriers of 288 threads; T = 40: one tile, 800 threads).  T = 44 and 36 have
+    tile_threads % 32 != 0: the one-launch plan must refuse them and the forced variant must fall back to one launch
+    per coarse colour -- same lattice either way"""
+    if kind in XS_KINDS and T % 8:
+        pytest.skip("xs1024 needs whole warps per tile")
+    S = L * L // 4
+    beta = 0.4
+    g, o = pkg.Rng(kind, S, 23), oracle.Rng(kind, S, 23)
+    g.set_variant("ising", 4)
+    sp = torch.empty(L * L, dtype=torch.int8, device="cuda")
+    pkg.ising_init_random(sp, L, 5)
+    sp_o = oracle.ising_init_random(L, 5)
+    for call in range(2):
+        l1 = pkg.rng_kernel_launches()
+        g.ising_sweep_multihit(sp, L, beta, sweeps, T, k)
+        assert pkg.rng_kernel_launches() - l1 == (1 if one_launch else 2 * sweeps)
+        o.ising_sweep_multihit(sp_o, L, beta, sweeps, T, k)
+        assert np.array_equal(sp.cpu().numpy(), sp_o), f"call {call}: lattice"
+    assert g.draws_done == o.draws_done == 2 * 4 * k * sweeps
+    if g.state_bytes():
+        assert np.array_equal(g.get_state(), o.get_state())
+    g.close()
+
+
 def test_ising_multihit_argument_errors():
     g = pkg.Rng(pkg.RNG_PHILOX4X32_10, 16, 1)
     sp = torch.ones(64, dtype=torch.int8, device="cuda")
