@@ -170,9 +170,13 @@ static cudaError_t xs_skip_matrices(int device, int levels, cudaStream_t st, uin
             b = t;
         }
         *launched += 138;
-        e = cudaStreamSynchronize(st);
+        // a launch that was refused is reported by cudaGetLastError, not by the synchronise: J[0] counts as
+        // valid (for every later handle of the process) only when both are clean
+        e = cudaGetLastError();
+        const cudaError_t es = cudaStreamSynchronize(st);
         cudaFree(tmp);
-        if (e != cudaSuccess) return e;
+        if (e == cudaSuccess) e = es;
+        if (e != cudaSuccess) return e; // levels stays 0: the next handle computes J[0] again
         c.levels = 1;
     }
     for (int k = c.levels; k < levels; k++) {
