@@ -176,12 +176,15 @@ __global__ void __launch_bounds__(WARPS * 32)
 // bandwidth, and a static "item += number of warps" split waits for the slowest SM -- the bare store pattern of
 // this kernel runs at 5.9 TB/s with the static split and at 7.0-7.3 TB/s with tickets, which is what a grid of
 // one-shot CTAs gets from the hardware's own CTA scheduler (B200 microbenchmark).
-// Tickets: *ticket counts up for the life of the handle; this launch owns [base, base + n_items) and every warp
-// takes exactly one ticket beyond that range before it leaves, so the host knows the next launch's base.
+// Tickets: *ticket is zero between launches.  Tickets 0 .. n_items-1 are the items; every warp takes exactly one
+// ticket beyond that range before it leaves, so the launch hands out n_items + (number of warps) tickets in all, and
+// the warp that draws the very last one knows that no other atomic on the counter is still to come: it puts the
+// counter back to zero.  A launch therefore depends on nothing the host remembers about earlier launches (a launch
+// that never runs, or a captured launch replayed any number of times, leaves the counter as it found it).
 template <int K, bool F32, int WARPS, int NT>
 __global__ void __launch_bounds__(WARPS * 32, 1)
     xs1024_fill_persistent_kernel(Gen g, uint64_t n, const __grid_constant__ CUtensorMap tmap,
-                                  unsigned long long *__restrict__ ticket, unsigned long long base)
+                                  unsigned long long *__restrict__ ticket)
 {
     extern __shared__ uint32_t xs_tiles_raw[];
     constexpr int P = 32 / K;
@@ -205,7 +208,10 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
     // items being written at any moment then spread over a proportionally wider address window).
     auto take = [&]() -> uint64_t { // warp-uniform next item
         unsigned long long v = 0ull;
-        if (lane == 0) v = atomicAdd(ticket, 1ull) - base;
+        if (lane == 0) {
+            v = atomicAdd(ticket, 1ull);
+            if (v == n_items + (uint64_t)gridDim.x * WARPS - 1ull) atomicExch(ticket, 0ull); // the last ticket of the launch
+        }
         return __shfl_sync(0xffffffffu, v, 0);
     };
     uint32_t w[K], wn[K];
@@ -382,12 +388,10 @@ static cudaError_t launch_xs_fill_persistent(const rng_handle &h, uint64_t n, bo
     cudaError_t e = cudaFuncSetAttribute(f32 ? kf : ku, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     unsigned long long *tk = (unsigned long long *)h.ticket;
-    if (f32) kf<<<(unsigned)grid, WARPS * 32, smem, st>>>(g, n, tm, tk, h.ticket_base);
-    else ku<<<(unsigned)grid, WARPS * 32, smem, st>>>(g, n, tm, tk, h.ticket_base);
+    if (f32) kf<<<(unsigned)grid, WARPS * 32, smem, st>>>(g, n, tm, tk);
+    else ku<<<(unsigned)grid, WARPS * 32, smem, st>>>(g, n, tm, tk);
     count_launch();
-    e = cudaGetLastError();
-    if (e == cudaSuccess) h.ticket_base += items + grid * WARPS; // every warp takes one ticket past the range
-    return e;
+    return cudaGetLastError();
 }
 
 // variant "xs1024" = K (0: default); variant "store": 0 = default, 1 = LDS/STG write-out, 2 = TMA tensor store;

@@ -50,10 +50,9 @@ struct rng_handle {
     void *staging;          // device staging for the *_host entry points
     uint64_t staging_bytes;
     int64_t *energy_scratch; // device, 1 x int64
-    // work tickets of the persistent fill kernels: a device counter that only counts up; a launch owns
-    // [ticket_base, ticket_base + its number of work items) and the host adds what the launch consumes
+    // work tickets of the persistent fill kernels: a device counter that is zero between launches (the warp
+    // that draws a launch's last ticket resets it, fill_xs1024.cu)
     uint64_t *ticket;            // device, 1 x uint64 (zero at rng_create)
-    mutable uint64_t ticket_base;
     uint32_t *ms_planes;     // device scratch of the multi-spin Ising path: two bit planes of L*L/64 words
     uint64_t ms_planes_bytes;
     unsigned long long *mh_mailbox; // device scratch of the one-launch multi-hit path: (L/T)^2 * 4 halo words

@@ -8,8 +8,6 @@ Rows are sampled at the start, the end and seeded random places (whole warp tile
 boundaries included); checksums / states are compared the same way.  C1 is small and is
 compared in full; the L = 8192 lattice is compared in full (the oracle needs ~1 s per sweep).
 """
-import os
-
 import numpy as np
 import pytest
 
@@ -107,25 +105,37 @@ def test_c3_xorwow_draw_reduce_full(big_buffer):
 
 
 def test_c4_xs1024_fill_calls_and_draw_full(big_buffer):
-    """C4: 2^24 streams.  Fill mode as bench.py runs it (calls of 64 draws into one buffer): the first
-    three calls on sampled instances; then draw mode (4096 draws) continuing the same handle."""
+    """C4: 2^24 streams.  Fill mode to the depth bench.py runs it: 64 consecutive calls of 64 draws into one buffer
+    on ONE handle (the persistent kernel's work-ticket counter and the Weyl index must carry across all of them);
+    sampled instances after calls 1, 2, 3, 32, 63 and 64, the generator state after call 64; then draw mode
+    (4096 draws) continuing the same handle."""
     cfg = W.C4_FILL
+    n_calls = 64
     g = pkg.Rng(cfg.kind, cfg.n_streams, cfg.seed)
     m = 128  # four instances
     shards = sample_shards(cfg.n_streams, m, 8, 3)
-    for call in (1, 2, 3):
+    for call in range(1, n_calls + 1):
+        if call in (32, 63):
+            big_buffer.zero_()  # a launch that wrote nothing would otherwise leave the previous call's rows behind
         g.fill_u32(big_buffer, cfg.n_per_stream)
-        check_fill_rows(cfg, big_buffer, call, m, shards)
+        if call in (1, 2, 3, 32, 63, 64):
+            check_fill_rows(cfg, big_buffer, call, m, shards)
+    assert g.draws_done == n_calls * cfg.n_per_stream
+    st = g.get_state()
+    for f in shards:
+        o = oracle.Rng(cfg.kind, m, cfg.seed, first=f, n_total=cfg.n_streams)
+        o.fill_u32(n_calls * cfg.n_per_stream)
+        assert np.array_equal(st[f:f + m], o.get_state()), f
     n_draw = W.C4_DRAW.n_per_stream
     g.draw_reduce(big_buffer, n_draw)
     red = big_buffer[:2 * cfg.n_streams].cpu().numpy().view(np.uint32).reshape(-1, 2)
     st = g.get_state()
     for f in shards[:5]:
         o = oracle.Rng(cfg.kind, m, cfg.seed, first=f, n_total=cfg.n_streams)
-        o.fill_u32(3 * cfg.n_per_stream)
+        o.fill_u32(n_calls * cfg.n_per_stream)
         assert np.array_equal(red[f:f + m].reshape(-1), o.draw_reduce(n_draw)), f
         assert np.array_equal(st[f:f + m], o.get_state()), f
-    assert g.draws_done == 3 * cfg.n_per_stream + n_draw
+    assert g.draws_done == n_calls * cfg.n_per_stream + n_draw
     g.close()
 
 
@@ -177,30 +187,13 @@ def _long_ising_call(kind, L, n_streams, n_sweeps, seed, lattice_seed, beta):
     g.close()
 
 
-@pytest.mark.parametrize("cfg", [W.C5B_PHILOX, W.C5B_XORWOW], ids=lambda c: c.name)
-def test_c5b_ising_L8192_100_sweeps_in_one_call(cfg):
-    """the whole 8192^2 lattice through ONE ising_sweep(n_sweeps = 100) call: the 100-entry energy trace, the final
-    lattice and the final generator state equal the oracle's (the oracle needs about a second per sweep)"""
-    _long_ising_call(cfg.kind, cfg.L, cfg.n_streams, 100, cfg.seed, cfg.lattice_seed, cfg.beta)
-
-
-@pytest.mark.parametrize("cfg", [W.C5B_PHILOX, W.C5B_XORWOW], ids=lambda c: c.name)
-def test_c5b_ising_1000_sweeps_in_one_call_L2048(cfg):
-    """the 1000-sweep single call that bench.py times (draw counter and Philox block index growing over 2000
-    half-sweeps, a 1000-entry trace, pack / unpack once around 1000 sweeps), on 1/16 of the lattice area with the
-    same number of sites per stream, so that the oracle finishes in about a minute"""
-    L = 2048
-    _long_ising_call(cfg.kind, L, cfg.n_streams // 16, 1000, cfg.seed, cfg.lattice_seed, cfg.beta)
-
-
-@pytest.mark.skipif(os.environ.get("RNG_B200_LONG_TESTS", "0") != "1",
-                    reason="3.5 minutes of oracle time: run with RNG_B200_LONG_TESTS=1 (green in round 2: 206 s on the "
-                           "GPU box); the same call is covered at L = 8192 x 100 sweeps and L = 2048 x 1000 sweeps above")
-def test_c5b_ising_L8192_1000_sweeps_exactly_as_benched():
-    """BASELINE config 5 to the letter: L = 8192, 1000 sweeps, ONE call (the call bench.py's C5b_xorwow times);
-    the 1000-entry energy trace, the final 64 MiB lattice and the final XORWOW states against the oracle
-    (about 3.5 minutes of oracle time, hence opt-in; the Philox variant of this call is covered at 100 sweeps above)"""
-    cfg = W.C5B_XORWOW
+@pytest.mark.parametrize("cfg", [W.C5B_XORWOW, W.C5B_PHILOX], ids=lambda c: c.name)
+def test_c5b_ising_L8192_1000_sweeps_exactly_as_benched(cfg):
+    """BASELINE config 5 to the letter: L = 8192, 1000 sweeps, ONE call -- the calls bench.py's C5b_xorwow and
+    C5b_philox time (draw counter and Philox block index growing over 2000 half-sweeps, pack / unpack once around
+    1000 sweeps).  The energy after sweeps 1, 2, 10, 100 and 1000, the whole 1000-entry trace,
+    the final 64 MiB lattice and the final generator states against the oracle.  About 3.5 minutes of oracle time
+    per generator; it replaces the 100-sweep and the L = 2048 x 1000-sweep cases of round 2, which it contains."""
     _long_ising_call(cfg.kind, cfg.L, cfg.n_streams, cfg.n_sweeps, cfg.seed, cfg.lattice_seed, cfg.beta)
 
 
