@@ -187,7 +187,8 @@ class ClockSampler:
             self._thr.join()
         s = sorted(self.samples)
         med = s[len(s) // 2] if s else None
-        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s)}
+        return {"sm_mhz": med, "sm_min_mhz": s[0] if s else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s), "sample_period_ms": self.period * 1e3}
 
 
 # ------------------------------------------------------------------------------------
@@ -370,10 +371,16 @@ def roofline(name: str, bound: str, alg_per_launch: float, sec_per_launch: float
     else:
         ach = alg_per_launch / sec_per_launch / 1e12
         peak = issue_peak_tinst(peaks["sm_max_mhz"])
+        # north_star asks for the ncu-MEASURED fraction of the issue peak: `frac` is smsp__issue_active of the
+        # committed capture of this workload's kernel (a static figure, not of this run); the hand-counted
+        # algorithmic instructions against the same peak are kept beside it as frac_algorithmic
         r = {"bound": "alu", "achieved": round(ach, 3), "peak": round(peak, 3), "unit": "Tinst/s",
-             "frac": round(ach / peak, 4), "basis": "algorithmic instruction count", "traffic": measured_traffic(name),
+             "frac": round(ach / peak, 4), "frac_algorithmic": round(ach / peak, 4),
+             "basis": "algorithmic instruction count", "traffic": measured_traffic(name),
              "peak_source": "148 SM x 4 SMSP x 32 lanes x sm_max_mhz issue slots"}
-        if ncu:
+        if ncu and ncu["issue_active_pct"] is not None:
+            r["frac"] = round(ncu["issue_active_pct"] / 100.0, 4)
+            r["basis"] = "frac = ncu smsp__issue_active (committed capture); achieved and frac_algorithmic = algorithmic instruction count"
             r["ncu_issue_active_pct"] = ncu["issue_active_pct"]
             r["ncu_binding_pipe"] = f"{ncu['binding_pipe']} {ncu['binding_pipe_pct']}%"
     r["ncu"] = ncu
@@ -541,6 +548,18 @@ def oracle_sample_rate(workload: str, target_s: float = 4.0, threads: int | None
                 break
         return {"value": L * L * sweeps / dt / 1e9, "unit": "flips/ns", "cores": cores, "kind": "oracle",
                 "sample": f"L={L} (1/16 of the 8192^2 lattice, same sites per stream), {sweeps} sweeps", "seconds": dt}
+    if workload.startswith("N2_seed"):
+        kind = oracle.XS1024W_SKIP if workload.endswith("skip") else oracle.XS1024W
+        n_streams, S = 1 << 24, 1 << 12
+        while True:  # seeding = creating the oracle's generator; grow the sample until it takes about target_s
+            t0 = time.perf_counter()
+            oracle.Rng(kind, S, W.MASTER_SEED)
+            dt = max(time.perf_counter() - t0, 1e-6)
+            if dt > target_s / 2 or S >= n_streams:
+                break
+            S = min(n_streams, S * 4)
+        return {"value": S / dt / 1e9, "unit": "Gstreams/s", "cores": cores, "kind": "oracle",
+                "sample": f"streams [0,{S}) of {n_streams} seeded (oracle rng_create)", "seconds": dt}
     cfgs = {"C2_u32": (W.C2, "fill_u32"), "C2_f32": (W.C2, "fill_f32"), "C1_u32": (W.C1, "fill_u32"),
             "C1_f32": (W.C1, "fill_f32"), "C1big_u32": (W.C1_BIG, "fill_u32"), "C3fill_u32": (W.C3_FILL, "fill_u32"),
             "C3_draw": (W.C3, "draw_reduce"), "C4_fill": (W.C4_FILL, "fill_u32"), "C4_draw": (W.C4_DRAW, "draw_reduce"),
@@ -700,11 +719,13 @@ SHORT_DESC = {
 }
 
 # BASELINE.json's own configs besides the headline: (workload, steps, warmup) of --suite baseline
-BASELINE_SUITE = [("C2_f32", 20, 3), ("C1_u32", 1000, 20), ("C1_f32", 1000, 20), ("C3_draw", 20, 3),
-                  ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1)]
+# plus row a1 (seeding) and the 4 GiB LCG64 supplement SURVEY.md 8(d) asks for beside C1
+BASELINE_SUITE = [("C2_f32", 20, 3), ("C1_u32", 1000, 20), ("C1_f32", 1000, 20), ("C1big_u32", 20, 3), ("C3_draw", 20, 3),
+                  ("C4_fill", 3, 1), ("C4_draw", 1, 1), ("C5b_philox", 1, 1), ("C5b_xorwow", 1, 1),
+                  ("N2_seed_xs1024_random", 5, 3), ("N2_seed_xs1024_skip", 5, 3)]
 
 
-def build_line(res: dict, args, world: int, cfg_info: dict, e2e=None, cpu=None, ceil=None, configs=None) -> dict:
+def build_line(res: dict, args, world: int, cfg_info: dict, e2e=None, cpu=None, ceil=None, configs=None, sustained=None) -> dict:
     """the ONE stdout JSON object of the b200 arm (kept compact: the driver reads the last few KB of stdout).
     `res` is run_job()'s result for the headline workload, `configs` the other workloads' results."""
     line = {
@@ -722,14 +743,21 @@ def build_line(res: dict, args, world: int, cfg_info: dict, e2e=None, cpu=None, 
         line["e2e"] = e2e
     if cpu:
         line["cpu_baseline"] = cpu
+    if sustained:
+        line["sustained"] = sustained
     if ceil:
         line["hbm_ceilings_measured_live"] = {k: round(v, 1) for k, v in ceil.items()}
     # only BASELINE.json's own configs ride on the line; --suite full's other workloads go to stderr / --dump
     own = {n for n, _, _ in BASELINE_SUITE}
-    rows = [[c["workload"], round(c["value"], 2), c["unit"], c["roofline"]["bound"], c["roofline"]["frac"]]
+    sig = lambda v: None if v is None else float(f"{v:.4g}")  # noqa: E731
+    rows = [[c["workload"], round(c["value"], 2), c["unit"], c["roofline"]["bound"], c["roofline"]["frac"],
+             c["roofline"].get("frac_vs_store_ceiling"), sig((c.get("cpu") or {}).get("value"))]
             for c in (configs or []) if c["workload"] in own]
     if rows:
-        line["configs_cols"] = ["workload", "value", "unit", "roofline_bound", "roofline_frac"]
+        # roofline_frac: hbm rows against the measured copy bandwidth (frac_vs_store: against the live memset
+        # ceiling -- a fill only writes); alu rows: ncu issue-active fraction.  cpu_oracle: the oracle on all host
+        # cores on a ~2 s sample of the same workload, same unit
+        line["configs_cols"] = ["workload", "value", "unit", "roofline_bound", "roofline_frac", "frac_vs_store", "cpu_oracle"]
         line["configs"] = rows
     return line
 
@@ -745,6 +773,8 @@ def main():
     ap.add_argument("--ising-sweeps", type=int, default=1000, help="sweeps per Ising step (config: 1000)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sustained-s", type=float, default=2.0,
+                    help="also run the headline step back to back for at least this many seconds (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dump", default=None, help="also write every workload's full result as a JSON list to this file")
     ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
@@ -793,6 +823,15 @@ def main():
 
     job = make_job(args.workload, rank, world, buf, args.ising_sweeps)
     res = run_job(job, args.steps, args.warmup, world, sample_clocks=True, dev_index=dev_index, store_gbs=store_gbs)
+    sustained = None
+    if world == 1 and args.sustained_s > 0 and not isinstance(job, (IsingJob, SeedJob)):
+        # the same step back to back for at least --sustained-s seconds: the power-limited regime beside the burst
+        n_sus = max(args.steps, int(args.sustained_s * 1e3 / max(res["ms_per_step"], 1e-3)) + 1)
+        rs = run_job(job, n_sus, 0, world, sample_clocks=True, dev_index=dev_index, store_gbs=store_gbs)
+        sustained = {"value": round(rs["value"], 2), "unit": rs["unit"], "steps": n_sus, "ms_per_step": round(rs["ms_per_step"], 5),
+                     "seconds": round(rs["ms_per_step"] * n_sus / 1e3, 2), "roofline_frac": rs["roofline"]["frac"],
+                     "frac_vs_store_ceiling": rs["roofline"].get("frac_vs_store_ceiling"), "clocks": rs.get("clocks")}
+        log(f"[bench] sustained {args.workload}: {rs['value']:.2f} {rs['unit']} over {sustained['seconds']} s, clocks {rs.get('clocks')}")
     e2e = None if args.no_e2e else run_e2e(job, args.e2e_steps, 1, world)
     cfg_info = {"desc": SHORT_DESC.get(args.workload, res["name"]),
                 "streams_per_gpu": getattr(getattr(job, "cfg", None), "n_streams", getattr(job, "n_local", None)),
@@ -816,6 +855,8 @@ def main():
         r = run_job(j, k, w, world, sample_clocks=False, dev_index=dev_index, store_gbs=store_gbs)
         j.close()
         r["workload"] = name
+        if rank == 0 and world == 1 and not args.no_cpu_baseline and suite == "baseline":
+            r["cpu"] = oracle_sample_rate(name, 2.0)
         configs.append(r)
         rl = r["roofline"]
         extra = f" (vs store ceiling {rl['frac_vs_store_ceiling']:.3f})" if "frac_vs_store_ceiling" in rl else \
@@ -824,7 +865,7 @@ def main():
             f"roofline {rl['bound']} {rl['frac']:.3f}{extra}")
 
     if rank == 0:
-        line = build_line(res, args, world, cfg_info, e2e, cpu, ceil if world == 1 else None, configs)
+        line = build_line(res, args, world, cfg_info, e2e, cpu, ceil if world == 1 else None, configs, sustained)
         if args.dump:
             with open(args.dump, "w") as f:
                 json.dump([dict(res, workload=args.workload)] + configs, f, indent=1)

@@ -41,6 +41,7 @@ def _stub_result(bench, workload, long_name, bound, unit="Gnum/s"):
          "ms_per_step": 0.67890123456789, "gpu_launches": 20, "dtype": "u32", "workload": workload,
          "clocks": {"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": ["sw_power_cap"], "samples": 4000}}
     r["roofline"] = bench.roofline(workload, bound, 4.3e9 if bound == "hbm" else 5e10, 6.8e-4, 7300.123)
+    r["cpu"] = {"value": 0.0123456789012, "unit": unit, "cores": 16, "kind": "oracle", "sample": "a sample", "seconds": 2.01}
     return r
 
 
@@ -63,7 +64,11 @@ def test_b200_line_is_one_compact_parseable_line_for_every_suite():
     for suite in ([], bench.BASELINE_SUITE, bench.SUITE):
         cfgs = [_stub_result(bench, n, n + "_some_long_name_2^22x4096", "alu" if ("draw" in n or n[0] in "T") else "hbm",
                              "flips/ns" if n[0] in "TC5" and "5b" in n or n[0] == "T" else "Gnum/s") for n, _, _ in suite]
-        line = json.dumps(bench.build_line(res, args, 1, info, e2e, cpu, ceil, cfgs))
+        sustained = {"value": 1432.12, "unit": "Gnum/s", "steps": 3196, "ms_per_step": 0.74912, "seconds": 2.39,
+                     "roofline_frac": 0.8912, "frac_vs_store_ceiling": 0.7801,
+                     "clocks": {"sm_mhz": 1755.0, "sm_min_mhz": 1687.0, "sm_max_mhz": 1965.0, "reasons": ["sw_power_cap"],
+                                "samples": 2390, "sample_period_ms": 1.0}}
+        line = json.dumps(bench.build_line(res, args, 1, info, e2e, cpu, ceil, cfgs, sustained))
         assert "\n" not in line and len(line) < 4096, len(line)
         d = json.loads(line)
         for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
@@ -82,7 +87,11 @@ def test_b200_line_is_one_compact_parseable_line_for_every_suite():
         for k in ("value", "unit", "cores", "kind", "sample", "single_thread"):
             assert k in d["cpu_baseline"], k
         assert d["cpu_baseline"]["single_thread"]["cores"] == 1
+        assert d["sustained"]["seconds"] >= 2.0 and d["sustained"]["clocks"]["samples"] > 1000
         if suite:
+            assert d["configs_cols"][-2:] == ["frac_vs_store", "cpu_oracle"]
+            assert all(row[-1] is not None and row[-1] > 0 for row in d["configs"])  # every BASELINE config has its CPU figure
+            assert {"N2_seed_xs1024_random", "N2_seed_xs1024_skip", "C1big_u32"} <= {row[0] for row in d["configs"]}  # row a1
             assert len(d["configs"]) <= 11 and all(len(row) == len(d["configs_cols"]) for row in d["configs"])
             own = {n for n, _, _ in bench.BASELINE_SUITE}
             assert {row[0] for row in d["configs"]} == own
@@ -92,8 +101,14 @@ def test_alu_roofline_leads_with_the_ncu_figures():
     sys.path.insert(0, ROOT)
     import bench
     rl = bench.roofline("C3_draw", "alu", 1.07e10, 3.5e-4)
-    assert rl["bound"] == "alu" and rl["basis"] == "algorithmic instruction count"
+    assert rl["bound"] == "alu" and rl["basis"].startswith("frac = ncu smsp__issue_active")
     assert rl["ncu"]["measured_in_this_run"] is False and rl["ncu_issue_active_pct"] > 0 and rl["ncu_binding_pipe"]
+    # north_star: the ncu-measured fraction of the issue peak leads; the hand count is kept beside it
+    assert abs(rl["frac"] - rl["ncu_issue_active_pct"] / 100.0) < 1e-3
+    assert abs(rl["frac_algorithmic"] - rl["achieved"] / rl["peak"]) < 1e-3
+    # a workload without a committed capture falls back to the hand count and says so
+    rl2 = bench.roofline("no_such_workload", "alu", 1.07e10, 3.5e-4)
+    assert rl2["frac"] == rl2["frac_algorithmic"] and rl2["basis"] == "algorithmic instruction count"
 
 
 def test_both_arms_name_the_workload_alike():
