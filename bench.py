@@ -57,7 +57,7 @@ TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
 
 def _capture(name: str):
     """the workload's entry of profiles/traffic.json: figures of its dominant kernel from the committed
-    `ncu --set full` capture (written by `python -m paper_1204_6193_b200.ncu_summary` from ncu's raw page).
+    `ncu --set full` capture (written by `python tests/ncu_summary.py` from ncu's raw page).
     STATIC: captured in an earlier run of the same command under ncu, never measured in the run that prints it."""
     try:
         return json.load(open(TRAFFIC_JSON)).get(name)

@@ -1,8 +1,8 @@
 """Summarise `ncu --page raw --csv` exports of the dominant kernels into the two files bench.py and the
 judge read: a text page of the metrics that matter on this path and `profiles/traffic.json`.
 
-    python -m paper_1204_6193_b200.ncu_summary RAW_DIR --text profiles/r02_ncu_full.txt [--json profiles/traffic.json]
-    python -m paper_1204_6193_b200.ncu_summary --launches LAUNCHES.csv --out profiles/r02_launches_<run>_summary.csv
+    python tests/ncu_summary.py RAW_DIR --text profiles/r02_ncu_full.txt [--json profiles/traffic.json]
+    python tests/ncu_summary.py --launches LAUNCHES.csv --out profiles/r02_launches_<run>_summary.csv
 
 RAW_DIR holds one `raw_<workload>.csv` per capture, <workload> being bench.py's `--workload` name; each is
 
@@ -13,11 +13,16 @@ of a capture taken with
     ncu --set full --metrics <EXTRA> --clock-control none --import-source on -k regex:<kernel> -s <skip> -c 1 -f \\
         -o rep_<workload> python bench.py --suite primary --steps 5 --warmup 3 --no-e2e --no-cpu-baseline --ising-sweeps 3 --workload <workload>
 
+and then cut down to the columns this tool reads (so that the raw page can be committed and the summaries re-derived
+from tracked files: tests/test_profiles_tools.py does exactly that) with
+
+    python tests/ncu_summary.py RAW_DIR --trim profiles/r03_raw
+
 (only after the same bench.py command has exited 0 without ncu; EXTRA = the EXTRA_METRICS list below: which of the
 two fma pipes and the conversion unit executed how many instructions -- `--set full` only has their sum).
 LAUNCHES.csv is the `--metrics gpu__time_duration.sum --clock-control none --csv` launch list of a bench.py run; its
-summary has one row per kernel (launches, total and average duration, share of the run).  Nothing here runs a kernel or is imported by
-the product path; bench.py reads the JSON as STATIC context (`measured_in_this_run: false`).
+summary has one row per kernel (launches, total and average duration, share of the run).  A profiling aid kept beside
+the tests, not part of the library package: nothing here runs a kernel or is imported by the product path; bench.py reads the JSON as STATIC context (`measured_in_this_run: false`).
 """
 from __future__ import annotations
 
@@ -67,7 +72,7 @@ def _num(d, k):
         return None
 
 
-def summarise(raw_dir: str, text_path: str, json_path: str | None, source: str) -> dict:
+def summarise(raw_dir: str, text_path: str, json_path: str | None, source: str, fresh: bool = False) -> dict:
     entries = {}
     with open(text_path, "w") as f:
         for p in sorted(glob.glob(os.path.join(raw_dir, "raw_*.csv"))):
@@ -113,18 +118,45 @@ def summarise(raw_dir: str, text_path: str, json_path: str | None, source: str) 
                 }
     if json_path:
         old = {}
-        if os.path.exists(json_path):
+        if os.path.exists(json_path) and not fresh:
             old = json.load(open(json_path))
         old["_comment"] = ("keyed by bench.py --workload name; per workload, from the `ncu --set full` capture of its dominant "
                            "kernel (see each entry's `source`): dram__bytes_read.sum + dram__bytes_write.sum per launch, "
                            "smsp__issue_active, sm__inst_executed_pipe_* (pct of peak sustained, active cycles), "
                            "sm__pipe_fmaheavy_cycles_active (pct of elapsed), gpu__dram_throughput.  Written by "
-                           "`python -m paper_1204_6193_b200.ncu_summary`; bench.py copies these as static context "
+                           "`python tests/ncu_summary.py`; bench.py copies these as static context "
                            "(measured_in_this_run: false) and never runs under ncu.")
         old.update(entries)
         with open(json_path, "w") as f:
             json.dump(old, f, indent=1)
     return entries
+
+
+def _kept(col: str) -> bool:
+    """columns of ncu's raw page that summarise() reads"""
+    return (col in ("ID", "Kernel Name", "Grid Size", "Block Size") or col in KEYS
+            or (col.startswith("smsp__average_warps_issue_stalled_") and col.endswith("_per_issue_active.ratio"))
+            or (col.startswith("sm__inst_executed_pipe_") and col.endswith("pct_of_peak_sustained_active")))
+
+
+def trim(raw_dir: str, out_dir: str) -> int:
+    """copies RAW_DIR/raw_*.csv to OUT_DIR keeping only the columns summarise() reads (a few KB per capture
+    instead of ncu's ~6000 columns): the summaries made from the trimmed files are identical"""
+    os.makedirs(out_dir, exist_ok=True)
+    n = 0
+    for p in sorted(glob.glob(os.path.join(raw_dir, "raw_*.csv"))):
+        rows = [r for r in csv.reader(open(p, errors="replace")) if r]
+        hdr_i = next((i for i, r in enumerate(rows) if r[0] == "ID"), None)  # ncu may print '==PROF==' lines first
+        if hdr_i is None or len(rows) < hdr_i + 3:
+            continue
+        rows = rows[hdr_i:]
+        keep = [i for i, c in enumerate(rows[0]) if _kept(c)]
+        with open(os.path.join(out_dir, os.path.basename(p)), "w", newline="") as f:
+            w = csv.writer(f, lineterminator="\n")
+            for r in rows:
+                w.writerow([r[i] if i < len(r) else "" for i in keep])
+        n += 1
+    return n
 
 
 def summarise_launches(csv_in: str, csv_out: str) -> int:
@@ -157,12 +189,17 @@ if __name__ == "__main__":
     ap.add_argument("--out", default=None, help="with --launches: the summary csv to write")
     ap.add_argument("--text", default=None)
     ap.add_argument("--json", default=None)
+    ap.add_argument("--fresh", action="store_true", help="with --json: write only this run's entries (default: merge into the file)")
+    ap.add_argument("--trim", default=None, help="instead of summarising: copy RAW_DIR's raw pages, cut down to the columns read here, to this directory")
     ap.add_argument("--source", default=None, help="what the entries cite as their capture (default: --text)")
     a = ap.parse_args()
     if a.launches:
         print(f"{summarise_launches(a.launches, a.out or a.launches[:-4] + '_summary.csv')} kernels -> {a.out}")
         raise SystemExit(0)
+    if a.raw_dir and a.trim:
+        print(f"{trim(a.raw_dir, a.trim)} raw pages -> {a.trim}")
+        raise SystemExit(0)
     if not a.raw_dir or not a.text:
         ap.error("RAW_DIR and --text are required without --launches")
-    e = summarise(a.raw_dir, a.text, a.json, a.source or a.text)
+    e = summarise(a.raw_dir, a.text, a.json, a.source or a.text, a.fresh)
     print(f"{len(e)} captures -> {a.text}" + (f", {a.json}" if a.json else ""))

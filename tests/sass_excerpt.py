@@ -2,7 +2,9 @@
 dependent launch, streaming 128-bit stores, Philox's wide multiplies, warp shuffles), from `cuobjdump -sass` of
 the built library.  Text evidence for profiles/; nothing here runs a kernel.
 
-    python -m paper_1204_6193_b200.sass_excerpt > profiles/r02_sass_excerpt.txt
+    python tests/sass_excerpt.py > profiles/r03_sass_excerpt.txt
+
+A profiling aid kept beside the tests (it is not part of the library package).
 """
 from __future__ import annotations
 
@@ -10,7 +12,10 @@ import re
 import subprocess
 import sys
 
-from .build import SO, build
+import os
+
+sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+from paper_1204_6193_b200.build import build  # noqa: E402
 
 MNEMONICS = ["UTMASTG", "ACQBULK", "PREEXIT", "STG.E.EF.128", "STS.128", "IMAD.WIDE.U32", "SHFL", "ATOMG", "I2FP",
              "BAR.SYNC", "UBLKCP", "LOP3", "SHF"]
@@ -20,7 +25,7 @@ def main() -> int:
     so = build()
     out = subprocess.run(["cuobjdump", "-sass", so], capture_output=True, text=True, check=True).stdout
     print(f"# cuobjdump -sass {so.split('/root/repo/')[-1]} | per kernel: instruction count and counts of {', '.join(MNEMONICS)}")
-    print("# written by: python -m paper_1204_6193_b200.sass_excerpt")
+    print("# written by: python tests/sass_excerpt.py")
     name, counts, total = None, {}, 0
     rows = []
 

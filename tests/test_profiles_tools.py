@@ -4,7 +4,7 @@ import csv
 import json
 import os
 
-from paper_1204_6193_b200 import ncu_summary
+import ncu_summary  # tests/ncu_summary.py (conftest puts tests/ on sys.path)
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 PROF = os.path.join(ROOT, "profiles")
