@@ -140,6 +140,14 @@ def mwc_multipliers(first: int, count: int) -> np.ndarray:
     return out
 
 
+def is_prime64(n: int) -> bool:
+    """the oracle's primality decision for n < 2^64 (trial division + Miller-Rabin)"""
+    L = lib()
+    L.orc_is_prime64.restype = C.c_int
+    L.orc_is_prime64.argtypes = [C.c_uint64]
+    return bool(L.orc_is_prime64(n))
+
+
 def xs1024_matpow2(k: int) -> np.ndarray:
     """M^(2^k) as a [1024, 32] uint32 bit matrix (row r = image of unit vector word r//32, bit r%32)"""
     out = np.empty((1024, 32), dtype=np.uint32)

@@ -319,26 +319,30 @@ int orc_mwc_is_multiplier(uint32_t a)
     uint64_t p = ((uint64_t)a << 32) - 1; /* a m - 1 */
     return a > 0 && orc_is_prime64((p - 1) / 2) && orc_is_prime64(p);
 }
-/* out[i] = multiplier number first + i, scanning down from 2^32 - 1.  returns 0, or -1 if the candidates run out */
+/* out[i] = multiplier number first + i, scanning down from 2^32 - 1.  returns 0, or -1 if the candidates run out.
+ * PAPER.md:97 as it reads: start at the top and work down one candidate at a time, counting those that qualify
+ * (plain sequential order, no chunking: slow -- about 1300 candidates per multiplier -- and meant to be).
+ * The list found so far is remembered for the life of the process, so that a later call continues the same scan
+ * where the last one stopped instead of starting again at the top (a memo of results; the order of work is the same). */
+static uint32_t *mwc_found;           /* multipliers number 0 .. mwc_n_found-1 */
+static uint64_t mwc_n_found, mwc_cap;
+static uint64_t mwc_next = 0xffffffffull; /* the next candidate a to look at */
 int orc_mwc_multipliers(uint64_t first, uint64_t count, uint32_t *out)
 {
-    /* the candidates are tested independently (in parallel, a chunk at a time) and then counted in order */
-    enum { CHUNK = 1 << 18 };
-    unsigned char *ok = (unsigned char *)malloc(CHUNK);
-    uint64_t k = 0, top = 0xffffffffull;
-    while (k < first + count && top >= 1) {
-        uint64_t nc = top < CHUNK ? top : CHUNK;
-#pragma omp parallel for schedule(dynamic, 1024)
-        for (uint64_t i = 0; i < nc; i++) ok[i] = (unsigned char)orc_mwc_is_multiplier((uint32_t)(top - i));
-        for (uint64_t i = 0; i < nc && k < first + count; i++)
-            if (ok[i]) {
-                if (k >= first) out[k - first] = (uint32_t)(top - i);
-                k++;
-            }
-        top -= nc;
+    const uint64_t need = first + count;
+    if (need > mwc_cap) {
+        uint64_t cap = mwc_cap ? mwc_cap : 1024;
+        while (cap < need) cap *= 2;
+        uint32_t *p = (uint32_t *)realloc(mwc_found, cap * sizeof *p);
+        if (!p) return -1;
+        mwc_found = p;
+        mwc_cap = cap;
     }
-    free(ok);
-    return k == first + count ? 0 : -1;
+    for (; mwc_n_found < need && mwc_next >= 1; mwc_next--)
+        if (orc_mwc_is_multiplier((uint32_t)mwc_next)) mwc_found[mwc_n_found++] = (uint32_t)mwc_next;
+    if (mwc_n_found < need) return -1;
+    memcpy(out, mwc_found + first, count * sizeof *out);
+    return 0;
 }
 
 /* G1: 32-bit LCG, eq.(1) with the constants of PAPER.md:46 */

@@ -8,6 +8,12 @@
  * It shares no code, header, table or constant generator with the CUDA path
  * under paper_1204_6193_b200/csrc/.  Only tests/, __graft_entry__.smoke() and
  * bench.py's cpu_baseline / --impl reference legs may load it.
+ * One place where oracle and kernel necessarily follow the same ALGORITHM is the
+ * primality test of the per-stream MWC multipliers (a kind outside SURVEY.md
+ * section 8): the paper prescribes Miller-Rabin and both sides use
+ * it, each in its own code.  Its pin therefore uses neither: tests/test_oracle_mwc.py
+ * accepts a prime only with a Pratt / Pocklington certificate and a composite only
+ * with a witness, and the scan below is the plain sequential one of the paper.
  *
  * Everything is integer arithmetic mod 2^32 / 2^64, so "precision" is exact;
  * the only floating point is the Ising acceptance table (double exp, rounded
