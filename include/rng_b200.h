@@ -280,11 +280,21 @@ uint64_t rng_state_bytes(int kind, uint64_t n_streams);
 int rng_get_state(rng_handle *h, void *h_buf, uint64_t bytes);
 int rng_set_state(rng_handle *h, const void *h_buf, uint64_t bytes);
 uint64_t rng_draws_done(const rng_handle *h);
+/* Sets the per-stream draw counter WITHOUT touching the device state.  For the counter-based kinds
+ * (PHILOX) the counter IS the position: any value repositions the streams.  For every stateful kind
+ * the counter must describe the device state or the two fall apart silently -- the Weyl index of
+ * XS1024W (term n of PAPER.md:236 is derived from draws_done), the half of the state LCG64_BOTH hands
+ * out next (draws_done & 1), and every "draws_done" a later checkpoint records.  So for those kinds
+ * call it only together with rng_set_state, with the draws_done that was read when that state was
+ * saved (checkpoint / resume); the library cannot check this and does not try. */
 int rng_set_draws_done(rng_handle *h, uint64_t draws_done);
 
-/* kernel-variant selection for measurements: name in {"xs1024", "xsfill", "ising", "store", "lcg", "cvt"},
- * value = variant index (0 = default).  Every variant of an operation produces
- * identical bits; see DESIGN.md section 6.  Unknown name/value: RNG_E_INVAL. */
+/* ---- TEST AND MEASUREMENT INTERFACE: not part of the product boundary --------
+ * Selects which of several bit-identical kernel variants a handle launches, so that tests can compare
+ * them with one another and bench runs can time them: name in {"xs1024", "xsfill", "ising", "store",
+ * "lcg", "cvt"}, value = variant index (0 = default, what every other caller gets and what bench.py
+ * times).  No result of any other entry point depends on it; applications have no reason to call it
+ * and it may change between versions.  See DESIGN.md section 6.  Unknown name/value: RNG_E_INVAL. */
 int rng_set_variant(rng_handle *h, const char *name, int value);
 
 /* number of kernels launched by this library in the calling process so far */

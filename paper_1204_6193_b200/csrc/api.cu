@@ -10,7 +10,6 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
-#include <vector>
 
 #include "internal.h"
 
@@ -469,11 +468,17 @@ int rng_get_state(rng_handle *h, void *h_buf, uint64_t bytes)
     CU(cudaDeviceSynchronize());
     const int wps = h->g.kind == RNG_XORWOW ? 6 : h->g.kind == RNG_MWC_MULTI ? 3 : 0; // words per stream of the SoA kinds
     if (wps) { // device layout w[k*S+s] -> canonical [s][k]
-        std::vector<uint32_t> tmp(h->g.S * wps);
-        CU(cudaMemcpy(tmp.data(), h->g.state, bytes, cudaMemcpyDeviceToHost));
+        uint32_t *tmp = new (std::nothrow) uint32_t[h->g.S * wps]; // nothing may throw across the C boundary
+        if (!tmp) return fail(RNG_E_NOMEM, "rng_get_state: host allocation of %llu bytes failed", (unsigned long long)bytes);
+        const cudaError_t e = cudaMemcpy(tmp, h->g.state, bytes, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) {
+            delete[] tmp;
+            return cuda_fail(e, "rng_get_state: cudaMemcpy");
+        }
         uint32_t *o = (uint32_t *)h_buf;
         for (uint64_t s = 0; s < h->g.S; s++)
             for (int k = 0; k < wps; k++) o[wps * s + k] = tmp[k * h->g.S + s];
+        delete[] tmp;
     } else {
         CU(cudaMemcpy(h_buf, h->g.state, bytes, cudaMemcpyDeviceToHost));
     }
@@ -490,11 +495,14 @@ int rng_set_state(rng_handle *h, const void *h_buf, uint64_t bytes)
     CU(cudaDeviceSynchronize());
     const int wps = h->g.kind == RNG_XORWOW ? 6 : h->g.kind == RNG_MWC_MULTI ? 3 : 0;
     if (wps) {
-        std::vector<uint32_t> tmp(h->g.S * wps);
+        uint32_t *tmp = new (std::nothrow) uint32_t[h->g.S * wps];
+        if (!tmp) return fail(RNG_E_NOMEM, "rng_set_state: host allocation of %llu bytes failed", (unsigned long long)bytes);
         const uint32_t *in = (const uint32_t *)h_buf;
         for (uint64_t s = 0; s < h->g.S; s++)
             for (int k = 0; k < wps; k++) tmp[k * h->g.S + s] = in[wps * s + k];
-        CU(cudaMemcpy(h->g.state, tmp.data(), bytes, cudaMemcpyHostToDevice));
+        const cudaError_t e = cudaMemcpy(h->g.state, tmp, bytes, cudaMemcpyHostToDevice);
+        delete[] tmp;
+        if (e != cudaSuccess) return cuda_fail(e, "rng_set_state: cudaMemcpy");
     } else {
         CU(cudaMemcpy(h->g.state, h_buf, bytes, cudaMemcpyHostToDevice));
     }
