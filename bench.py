@@ -776,6 +776,8 @@ def main():
     ap.add_argument("--sustained-s", type=float, default=2.0,
                     help="also run the headline step back to back for at least this many seconds (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant", default=None, help="NAME=VALUE: time a non-default kernel variant of the headline "
+                    "workload (rng_set_variant, the library's test and measurement interface), e.g. xs1024=33")
     ap.add_argument("--dump", default=None, help="also write every workload's full result as a JSON list to this file")
     ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
                     help="torch.distributed backend for N > 1 (nccl: one rank per GPU; gloo only for flow tests)")
@@ -822,6 +824,11 @@ def main():
     store_gbs = ceil["memset_write_gbs"]
 
     job = make_job(args.workload, rank, world, buf, args.ising_sweeps)
+    variant = None
+    if args.variant:  # measurements of the non-default kernel variants (bit-identical)
+        vn, vv = args.variant.split("=")
+        job.rng.set_variant(vn, int(vv))
+        variant = {vn: int(vv)}
     res = run_job(job, args.steps, args.warmup, world, sample_clocks=True, dev_index=dev_index, store_gbs=store_gbs)
     sustained = None
     if world == 1 and args.sustained_s > 0 and not isinstance(job, (IsingJob, SeedJob)):
@@ -837,6 +844,8 @@ def main():
                 "streams_per_gpu": getattr(getattr(job, "cfg", None), "n_streams", getattr(job, "n_local", None)),
                 "l2": "64 MiB lattice is L2-resident by design (DESIGN.md s7)" if isinstance(job, IsingJob)
                 else "4 GiB output per step > 126 MB L2, no flush needed"}
+    if variant:
+        cfg_info["variant"] = variant
     job.close()
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

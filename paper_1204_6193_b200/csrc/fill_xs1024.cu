@@ -316,6 +316,55 @@ __global__ void __launch_bounds__(THREADS) xs1024_draw_kernel(Gen g, uint32_t *_
     }
 }
 
+// The A/B partner of xs1024_draw_kernel<1, ..>: the same one-word-per-thread layout with the exchange through
+// shared memory, i.e. the paper's Listing 1 as it has to be written since Volta -- its padded
+// per-warp array (zeros on both sides stand for the words shifted in from outside the state),
+// with __syncwarp() wherever the listing relies on implicit warp synchrony and `volatile` (footnote 3,
+// PAPER.md:189, expects shuffles to replace it).  Variant "xs1024" = 33, draw mode only; same bits as every other
+// layout.  Measured against the shuffle form in DESIGN.md section 8.
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS) xs1024_draw_smem_kernel(Gen g, uint32_t *__restrict__ out, uint64_t n)
+{
+    constexpr int PAD = 11, ROW = PAD + 32 + PAD;
+    __shared__ uint32_t rows[THREADS / 32][ROW];
+    const int lane = threadIdx.x & 31;
+    const uint64_t wg = ((uint64_t)blockIdx.x * THREADS + threadIdx.x) >> 5;
+    const uint64_t s0 = wg * 32ull;
+    if (s0 >= g.S) return; // warp-uniform (S is a multiple of 32)
+    uint32_t *r = rows[threadIdx.x >> 5] + PAD; // r[-11 .. -1] and r[32 .. 42] stay zero
+    if (lane < PAD) r[-1 - lane] = 0u, r[32 + lane] = 0u;
+    uint32_t *state = (uint32_t *)g.state;
+    uint32_t v = state[s0 + lane], x = 0u, sum = 0u, wsum = 0u;
+    r[lane] = v;
+    __syncwarp();
+    uint32_t nupd = (uint32_t)g.draws_done;
+#pragma unroll 1
+    for (uint64_t i = 0; i < n; i++) {
+        uint32_t a = r[lane + 10], b = r[lane + 11]; // A: X ^= X << 329
+        __syncwarp();
+        v ^= (a << 9) | (b >> 23);
+        r[lane] = v;
+        __syncwarp();
+        a = r[lane - 10], b = r[lane - 11];          // B: X ^= X >> 347
+        __syncwarp();
+        v ^= (a >> 27) | (b << 5);
+        r[lane] = v;
+        __syncwarp();
+        a = r[lane + 10], b = r[lane + 11];          // C: X ^= X << 344
+        __syncwarp();
+        v ^= (a << 24) | (b >> 8);
+        r[lane] = v;
+        __syncwarp();
+        nupd++;
+        const uint32_t wt = xs1024_weyl_term(nupd);
+        wsum += wt;
+        x ^= wt + v;
+        sum += v;
+    }
+    state[s0 + lane] = v;
+    reinterpret_cast<uint2 *>(out)[s0 + lane] = make_uint2(x, sum + wsum);
+}
+
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -453,6 +502,13 @@ cudaError_t launch_xs1024_draw(const rng_handle &h, uint32_t *d_out, uint64_t n,
     // the API asks for 8-byte alignment only; K >= 2 stores 16-byte vectors
     if (((uintptr_t)d_out & 15u) != 0u) return launch_xs_draw<1, 256>(h.g, d_out, n, st);
     switch (h.var_xs1024) {
+    case 33: { // K = 1 with the paper's shared-memory exchange (measurement partner of case 1)
+        const uint64_t grid = (h.g.S / 32 + 7) / 8;
+        if (grid > 0x7fffffffull) return cudaErrorInvalidConfiguration;
+        xs1024_draw_smem_kernel<256><<<(unsigned)grid, 256, 0, st>>>(h.g, d_out, n);
+        count_launch();
+        return cudaGetLastError();
+    }
     case 1: return launch_xs_draw<1, 256>(h.g, d_out, n, st);
     case 2: return launch_xs_draw<2, 256>(h.g, d_out, n, st);
     case 4: return launch_xs_draw<4, 256>(h.g, d_out, n, st);

@@ -304,6 +304,24 @@ def test_xs1024_lane_layouts_are_one_generator(K, store):
         g.close()
 
 
+def test_xs1024_shared_memory_exchange_is_the_same_generator():
+    """the paper's Listing 1 with __syncwarp (variant "xs1024" = 33, draw mode): same checksums and final state as the
+    oracle, i.e. as the shuffle layouts; several CTAs, a ragged last CTA, continuation across calls and variants"""
+    for kind in XS_KINDS:
+        S = 32 * 37
+        g, o = pkg.Rng(kind, S, 4), oracle.Rng(kind, S, 4)
+        g.set_variant("xs1024", 33)
+        red = dev_u32(2 * S)
+        for n in (1, 100, 257):
+            g.draw_reduce(red, n)
+            assert np.array_equal(host(red, 2 * S), o.draw_reduce(n)), n
+        assert np.array_equal(g.get_state(), o.get_state())
+        g.set_variant("xs1024", 1)          # the shuffle form of the same layout continues the same streams
+        g.draw_reduce(red, 64)
+        assert np.array_equal(host(red, 2 * S), o.draw_reduce(64))
+        g.close()
+
+
 @pytest.mark.parametrize("xsfill", [0, 1, 2, 3], ids=["by_row_length", "one_shot_ctas", "tickets_1_tile", "tickets_2_tiles"])
 @pytest.mark.parametrize("K", [1, 2, 4, 8, 16])
 def test_xs1024_fill_schedules_are_one_generator(K, xsfill):
